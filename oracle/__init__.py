@@ -1,0 +1,162 @@
+"""CPU oracle for the second-order Trotter-Suzuki step -- TEST INFRASTRUCTURE ONLY.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  The product path
+(``paper_1208_2407_b200``) never does, and this package never imports the product.
+
+The arithmetic lives in ``ts_oracle.c`` (plain C, double precision, the paper's operator
+sequence written out; citations there).  This file only builds it with gcc, loads it with
+ctypes and marshals numpy arrays.  ``window_evolve`` is the causal-window oracle of
+SURVEY.md 8(c): the same C routine run on a cut-out whose margin exceeds the light cone
+(2 sites per step when the window origin is even), so it is exact on the interior.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "ts_oracle.c"
+_LIB = _HERE / "libts_oracle.so"
+_lib = None
+
+_D = ctypes.POINTER(ctypes.c_double)
+
+
+def build(force: bool = False) -> Path:
+    """Compile ts_oracle.c -> libts_oracle.so (gcc -O2 -fopenmp, no fast-math)."""
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+        tmp = _LIB.with_suffix(f".so.tmp{os.getpid()}")
+        cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-Wall", "-Wextra",
+               "-o", str(tmp), str(_SRC)]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(str(_LIB))
+        i64, dbl, i32 = ctypes.c_int64, ctypes.c_double, ctypes.c_int
+        lib.oracle_sweep.argtypes = [_D, _D, i64, i64, i32, i32, dbl, dbl, i32]
+        lib.oracle_sweep.restype = None
+        lib.oracle_phase.argtypes = [_D, _D, i64, i64, _D, _D]
+        lib.oracle_phase.restype = None
+        lib.oracle_step.argtypes = [_D, _D, i64, i64, dbl, dbl, dbl, dbl, _D, _D, i32]
+        lib.oracle_step.restype = None
+        lib.oracle_evolve.argtypes = [_D, _D, i64, i64, dbl, dbl, dbl, dbl, _D, _D, i32, i64]
+        lib.oracle_evolve.restype = None
+        lib.oracle_norm2.argtypes = [_D, _D, i64, i64]
+        lib.oracle_norm2.restype = dbl
+        lib.oracle_num_threads.argtypes = []
+        lib.oracle_num_threads.restype = i32
+        lib.oracle_set_num_threads.argtypes = [i32]
+        lib.oracle_set_num_threads.restype = None
+        _lib = lib
+    return _lib
+
+
+def _plane(a: np.ndarray) -> np.ndarray:
+    if a.dtype != np.float64 or a.ndim != 2 or not a.flags.c_contiguous or not a.flags.writeable:
+        raise ValueError("oracle planes must be writable C-contiguous float64 [ny][nx] arrays")
+    return a
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(_D)
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    _load().oracle_set_num_threads(int(n))
+
+
+def sweep(re, im, axis: int, parity: int, a: float, b: float, periodic: bool) -> None:
+    """In place: one checkerboard sweep (axis 0 = x, 1 = y; parity 0 = even, 1 = odd)."""
+    _plane(re), _plane(im)
+    ny, nx = re.shape
+    _load().oracle_sweep(_ptr(re), _ptr(im), nx, ny, axis, parity, a, b, int(bool(periodic)))
+
+
+def phase(re, im, pot_re, pot_im) -> None:
+    """In place: psi <- psi * (pot_re + i pot_im)."""
+    _plane(re), _plane(im)
+    ny, nx = re.shape
+    pot_re = np.ascontiguousarray(pot_re, dtype=np.float64)
+    pot_im = np.ascontiguousarray(pot_im, dtype=np.float64)
+    assert pot_re.shape == re.shape and pot_im.shape == re.shape
+    _load().oracle_phase(_ptr(re), _ptr(im), nx, ny, _ptr(pot_re), _ptr(pot_im))
+
+
+def evolve(re, im, a_half, b_half, a_full, b_full, pot=None, periodic=False, n_steps=1) -> None:
+    """In place: n_steps second-order steps.  pot = None or (pot_re, pot_im) float64 planes."""
+    _plane(re), _plane(im)
+    ny, nx = re.shape
+    if im.shape != re.shape:
+        raise ValueError("re/im shape mismatch")
+    if periodic and (nx % 2 or ny % 2):
+        raise ValueError("periodic needs even nx, ny (an odd ring cannot be 2-coloured)")
+    pr = pi = None
+    if pot is not None:
+        pr = np.ascontiguousarray(pot[0], dtype=np.float64)
+        pi = np.ascontiguousarray(pot[1], dtype=np.float64)
+        assert pr.shape == re.shape and pi.shape == re.shape
+    _load().oracle_evolve(_ptr(re), _ptr(im), nx, ny, a_half, b_half, a_full, b_full,
+                          _ptr(pr), _ptr(pi), int(bool(periodic)), int(n_steps))
+
+
+def norm2(re, im) -> float:
+    re = np.ascontiguousarray(re, dtype=np.float64)
+    im = np.ascontiguousarray(im, dtype=np.float64)
+    ny, nx = re.shape
+    return float(_load().oracle_norm2(_ptr(re), _ptr(im), nx, ny))
+
+
+def window_evolve(fetch, nx: int, ny: int, x0: int, y0: int, w: int, h: int,
+                  a_half, b_half, a_full, b_full, periodic: bool, n_steps: int,
+                  fetch_pot=None):
+    """Causal-window oracle: exact result on the w x h window at (x0, y0) of an nx x ny lattice.
+
+    ``fetch(ys, xs) -> (re, im)`` returns the INITIAL state (float64) at the index grids
+    ``ys[:, None], xs[None, :]`` (already reduced modulo the lattice for periodic);
+    ``fetch_pot`` likewise returns (pot_re, pot_im).  The window is grown by a margin of
+    2*n_steps + 2 sites per side (the dependency cone is 2 sites per step when
+    the cut starts on an even coordinate), snapped to even coordinates, and clipped at real
+    closed edges so those coincide with the cut-out's own closed edges.  The cut-out is evolved
+    as a CLOSED lattice by the same C routine; the margin is discarded.
+    """
+    m = 2 * n_steps + 2
+    lo_x, hi_x = x0 - m, x0 + w + m
+    lo_y, hi_y = y0 - m, y0 + h + m
+    lo_x -= lo_x % 2
+    lo_y -= lo_y % 2
+    hi_x += hi_x % 2
+    hi_y += hi_y % 2
+    if periodic:
+        if hi_x - lo_x >= nx or hi_y - lo_y >= ny:
+            raise ValueError("window + margin wraps onto itself; use the full oracle")
+        xs = np.arange(lo_x, hi_x) % nx
+        ys = np.arange(lo_y, hi_y) % ny
+    else:
+        lo_x, lo_y = max(lo_x, 0), max(lo_y, 0)
+        hi_x, hi_y = min(hi_x, nx), min(hi_y, ny)
+        xs = np.arange(lo_x, hi_x)
+        ys = np.arange(lo_y, hi_y)
+    re, im = fetch(ys, xs)
+    re = np.array(re, dtype=np.float64, order="C")
+    im = np.array(im, dtype=np.float64, order="C")
+    pot = None
+    if fetch_pot is not None:
+        pot = fetch_pot(ys, xs)
+    evolve(re, im, a_half, b_half, a_full, b_full, pot=pot, periodic=False, n_steps=n_steps)
+    ox, oy = x0 - lo_x, y0 - lo_y
+    return re[oy:oy + h, ox:ox + w].copy(), im[oy:oy + h, ox:ox + w].copy()
