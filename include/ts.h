@@ -1,0 +1,115 @@
+/*
+ * ts.h -- C ABI of libts: second-order Trotter-Suzuki time step for one particle on a 2-D
+ * lattice, NVIDIA B200 (sm_100a).  Plain pointers and sizes only; no C++/torch types.
+ *
+ * What it computes (PAPER.md = the paper's text; readings R1..R13 are listed in DESIGN.md):
+ *   The lattice Hamiltonian is split into a diagonal part H0 and, per axis, an even-pair and an
+ *   odd-pair part.  The exponential of a pair part is a set of
+ *   independent 2x2 plane rotations M = [[a, i b],[i b, a]].  One time step is
+ *   the symmetrised second-order product U2 = U1^T U1 (Eq. 3), here
+ *
+ *      Xe(h) Xo(h) Ye(h) [ Yo(f) | Yo(h) P Yo(h) ] Ye(h) Xo(h) Xe(h)       applied left to right,
+ *
+ *   X/Y = horizontal/vertical, e/o = even pairs (2k,2k+1) / odd pairs (2k+1,2k+2),
+ *   (h) = half-angle coefficients (a_half, b_half), (f) = full-angle (a_full, b_full),
+ *   P = multiplication by the unit-modulus potential phase exp(-i V dt).
+ *
+ * Data layout: the wavefunction is two dense planes psi_re[ny][nx], psi_im[ny][nx] (x fastest,
+ * element (x, y) at y*nx + x) of the plan's dtype, in DEVICE memory, each 16-byte aligned and
+ * non-overlapping.  pot_phase is 2*ny*nx elements of the same dtype in DEVICE memory: plane 0 =
+ * Re = cos(V dt), plane 1 = Im = -sin(V dt).
+ *
+ * Every function returns TS_OK (0) or an error code; nothing is enqueued when an error is
+ * returned by argument validation.  ts_last_error() gives a thread-local text for the last
+ * failure on the calling thread.  No exceptions cross this boundary.
+ */
+#ifndef TS_H_
+#define TS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ts_plan ts_plan;               /* opaque; owned by the library */
+
+enum { TS_F32 = 0, TS_F64 = 1 };              /* dtype of psi planes and pot_phase */
+enum { TS_CLOSED = 0, TS_PERIODIC = 1 };      /* boundary, same on both axes */
+enum { TS_OK = 0, TS_EINVAL = 1, TS_EUNSUPPORTED = 2, TS_EALLOC = 3, TS_ECUDA = 4 };
+
+/*
+ * ts_plan_create -- describe a lattice (L x L mesh; here nx x ny).
+ *   nx, ny    lattice extent, >= 1, nx*ny < 2^62.
+ *   dtype     TS_F32 or TS_F64.
+ *   boundary  TS_CLOSED: pairs crossing the edge are omitted, unpaired sites are unchanged in
+ *             that sweep (the zero 1x1 blocks of the printed H1/H2);
+ *             TS_PERIODIC: the wrap pair (n-1, 0) belongs to the odd sweep; needs nx, ny even.
+ * Returns a plan bound to the CUDA device current at the call, or NULL (see ts_last_error()).
+ * The plan owns all scratch (second state buffer for the double-buffered fused kernel,
+ * PAPER.md:109; reduction workspace); scratch is allocated on first use and freed by
+ * ts_plan_destroy.  A plan may be reused across calls and streams, but not concurrently.
+ */
+ts_plan* ts_plan_create(int64_t nx, int64_t ny, int dtype, int boundary);
+
+/*
+ * ts_evolve -- psi <- U2^n_steps psi, in place from the caller's view (Eq. 3).
+ *   psi_re, psi_im   DEVICE pointers, ny*nx elements each, 16-byte aligned, caller-owned.
+ *   a_half, b_half   cos, sin of theta/2, theta = dt*|V_tunnel|/hbar.
+ *   a_full, b_full   cos, sin of theta; used by the middle sweep when pot_phase is NULL.
+ *                    Both pairs must be finite with |a^2 + b^2 - 1| <= 1e-6.  The sign of b is
+ *                    the caller's: (b -> -b, pot_phase -> conj) is the time-reversed step.
+ *   pot_phase_or_null  NULL: 7-stage step.  Else DEVICE pointer to 2*ny*nx elements: 9-stage
+ *                    step with the phase at the centre (a_full, b_full validated but unused).
+ *   n_steps          >= 0; 0 is a no-op.
+ *   cuda_stream      cudaStream_t passed as void* (NULL = legacy default stream).
+ * Work is enqueued on the stream; the call does not synchronise.  The plan's scratch buffer is
+ * in use until that work completes.
+ * Errors: TS_EINVAL (NULL/misaligned/overlapping pointers, bad coefficients, n_steps < 0),
+ * TS_EALLOC (scratch allocation), TS_ECUDA (launch failure; text in ts_last_error()).
+ */
+int ts_evolve(ts_plan* plan, void* psi_re, void* psi_im,
+              double a_half, double b_half, double a_full, double b_full,
+              const void* pot_phase_or_null, int64_t n_steps, void* cuda_stream);
+
+/*
+ * ts_norm -- squared norm sum |psi|^2, accumulated in double for either dtype.
+ *   psi_re, psi_im   DEVICE pointers as above (read only).
+ *   out_norm2_host   HOST pointer to one double, written before the call returns.
+ * Enqueues on cuda_stream and synchronises that stream.
+ */
+int ts_norm(ts_plan* plan, const void* psi_re, const void* psi_im,
+            double* out_norm2_host, void* cuda_stream);
+
+/*
+ * ts_evolve_host -- the same operation for HOST-resident planes (pageable or pinned): copies
+ * psi (and pot_phase when given) to plan-owned device buffers, runs ts_evolve, copies psi
+ * back, and synchronises.  This is the end-to-end entry measured by bench.py's "e2e".
+ */
+int ts_evolve_host(ts_plan* plan, void* psi_re_host, void* psi_im_host,
+                   double a_half, double b_half, double a_full, double b_full,
+                   const void* pot_phase_host_or_null, int64_t n_steps);
+
+/*
+ * ts_plan_set_option -- tuning knobs, all optional.  Unknown names give TS_EINVAL.
+ *   "path"         0 = auto, 1 = generic per-sweep kernels only, 2 = fused kernel required
+ *                  (ts_evolve then returns TS_EUNSUPPORTED for shapes the fused kernel cannot take).
+ *   "fuse_steps"   steps fused per pass over HBM (1..TS_MAX_FUSE), 0 = auto.
+ *   "seg_rows"     rows of output per streaming segment of the fused kernel, 0 = auto.
+ */
+int ts_plan_set_option(ts_plan* plan, const char* name, int64_t value);
+
+/* ts_plan_get_info -- read back what the last ts_evolve used:
+ *   "fused" (0/1), "fuse_steps", "passes", "launches" (kernels + copies enqueued), "seg_rows". */
+int ts_plan_get_info(const ts_plan* plan, const char* name, int64_t* out_value);
+
+int ts_plan_destroy(ts_plan* plan);           /* NULL is accepted (no-op, TS_OK) */
+
+const char* ts_last_error(void);              /* never NULL; "" if no failure yet */
+
+#define TS_MAX_FUSE 4
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TS_H_ */

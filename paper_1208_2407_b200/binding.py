@@ -1,0 +1,157 @@
+"""ctypes binding of libts.so -- argument marshalling only; every step of the path runs in the
+CUDA kernels behind include/ts.h.  torch is used for device memory and stream handles."""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+TS_F32, TS_F64 = 0, 1
+TS_CLOSED, TS_PERIODIC = 0, 1
+TS_OK, TS_EINVAL, TS_EUNSUPPORTED, TS_EALLOC, TS_ECUDA = 0, 1, 2, 3, 4
+TS_MAX_FUSE = 4
+
+_LIB_PATH = Path(__file__).resolve().parent / "libts.so"
+_lib = None
+
+SYMBOLS = ["ts_plan_create", "ts_evolve", "ts_norm", "ts_evolve_host", "ts_plan_set_option",
+           "ts_plan_get_info", "ts_plan_destroy", "ts_last_error"]
+
+
+class TsError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libts error {code}: {msg}")
+        self.code = code
+
+
+def lib():
+    """Load libts.so; there is no fallback -- a missing library is an error."""
+    global _lib
+    if _lib is None:
+        if not _LIB_PATH.exists():
+            raise RuntimeError(f"{_LIB_PATH} is missing: run `python -m paper_1208_2407_b200.build` "
+                               "(there is no CPU fallback)")
+        L = ctypes.CDLL(str(_LIB_PATH))
+        vp, i64, dbl, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int
+        L.ts_plan_create.argtypes = [i64, i64, i32, i32]
+        L.ts_plan_create.restype = vp
+        L.ts_evolve.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp, i64, vp]
+        L.ts_evolve.restype = i32
+        L.ts_norm.argtypes = [vp, vp, vp, ctypes.POINTER(dbl), vp]
+        L.ts_norm.restype = i32
+        L.ts_evolve_host.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp, i64]
+        L.ts_evolve_host.restype = i32
+        L.ts_plan_set_option.argtypes = [vp, ctypes.c_char_p, i64]
+        L.ts_plan_set_option.restype = i32
+        L.ts_plan_get_info.argtypes = [vp, ctypes.c_char_p, ctypes.POINTER(i64)]
+        L.ts_plan_get_info.restype = i32
+        L.ts_plan_destroy.argtypes = [vp]
+        L.ts_plan_destroy.restype = i32
+        L.ts_last_error.argtypes = []
+        L.ts_last_error.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def last_error() -> str:
+    return lib().ts_last_error().decode()
+
+
+def _check(rc):
+    if rc != TS_OK:
+        raise TsError(rc, last_error())
+
+
+def _dtype_code(torch_dtype):
+    import torch
+    if torch_dtype == torch.float32:
+        return TS_F32
+    if torch_dtype == torch.float64:
+        return TS_F64
+    raise TypeError("psi planes must be float32 or float64")
+
+
+def _stream_handle(stream):
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+class Plan:
+    """ts_plan_create / ts_plan_destroy.  boundary: "closed" or "periodic"."""
+
+    def __init__(self, nx: int, ny: int, dtype, boundary: str = "closed"):
+        self.nx, self.ny = int(nx), int(ny)
+        self.dtype = dtype
+        b = {"closed": TS_CLOSED, "periodic": TS_PERIODIC}[boundary]
+        self._h = lib().ts_plan_create(self.nx, self.ny, _dtype_code(dtype), b)
+        if not self._h:
+            raise TsError(TS_EINVAL, last_error())
+
+    def set_option(self, name: str, value: int):
+        _check(lib().ts_plan_set_option(self._h, name.encode(), int(value)))
+
+    def info(self, name: str) -> int:
+        out = ctypes.c_int64(0)
+        _check(lib().ts_plan_get_info(self._h, name.encode(), ctypes.byref(out)))
+        return out.value
+
+    def _planes(self, re, im):
+        if re.dtype != self.dtype or im.dtype != self.dtype:
+            raise TypeError("plane dtype differs from the plan's")
+        if tuple(re.shape) != (self.ny, self.nx) or tuple(im.shape) != (self.ny, self.nx):
+            raise ValueError("planes must have shape [ny][nx]")
+        if not (re.is_contiguous() and im.is_contiguous()):
+            raise ValueError("planes must be contiguous")
+
+    def evolve(self, psi_re, psi_im, a_half, b_half, a_full, b_full, pot_phase=None,
+               n_steps=1, stream=None):
+        """ts_evolve on CUDA tensors, in place, asynchronous on `stream` (default: current)."""
+        self._planes(psi_re, psi_im)
+        if not (psi_re.is_cuda and psi_im.is_cuda):
+            raise ValueError("evolve takes CUDA tensors; use evolve_host for host tensors")
+        pot = None
+        if pot_phase is not None:
+            if pot_phase.dtype != self.dtype or tuple(pot_phase.shape) != (2, self.ny, self.nx) \
+                    or not pot_phase.is_contiguous() or not pot_phase.is_cuda:
+                raise ValueError("pot_phase must be a contiguous CUDA tensor [2][ny][nx]")
+            pot = ctypes.c_void_p(pot_phase.data_ptr())
+        _check(lib().ts_evolve(self._h, ctypes.c_void_p(psi_re.data_ptr()),
+                               ctypes.c_void_p(psi_im.data_ptr()), a_half, b_half, a_full, b_full,
+                               pot, int(n_steps), _stream_handle(stream)))
+
+    def evolve_host(self, psi_re, psi_im, a_half, b_half, a_full, b_full, pot_phase=None,
+                    n_steps=1):
+        """ts_evolve_host on HOST tensors (pinned or pageable), in place, synchronous."""
+        self._planes(psi_re, psi_im)
+        if psi_re.is_cuda or psi_im.is_cuda:
+            raise ValueError("evolve_host takes host tensors")
+        pot = None
+        if pot_phase is not None:
+            if pot_phase.dtype != self.dtype or tuple(pot_phase.shape) != (2, self.ny, self.nx) \
+                    or not pot_phase.is_contiguous() or pot_phase.is_cuda:
+                raise ValueError("pot_phase must be a contiguous host tensor [2][ny][nx]")
+            pot = ctypes.c_void_p(pot_phase.data_ptr())
+        _check(lib().ts_evolve_host(self._h, ctypes.c_void_p(psi_re.data_ptr()),
+                                    ctypes.c_void_p(psi_im.data_ptr()), a_half, b_half, a_full,
+                                    b_full, pot, int(n_steps)))
+
+    def norm(self, psi_re, psi_im, stream=None) -> float:
+        """ts_norm: sum |psi|^2 as a host float (synchronises the stream)."""
+        self._planes(psi_re, psi_im)
+        out = ctypes.c_double(0.0)
+        _check(lib().ts_norm(self._h, ctypes.c_void_p(psi_re.data_ptr()),
+                             ctypes.c_void_p(psi_im.data_ptr()), ctypes.byref(out),
+                             _stream_handle(stream)))
+        return out.value
+
+    def destroy(self):
+        if self._h:
+            lib().ts_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

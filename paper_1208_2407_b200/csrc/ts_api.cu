@@ -1,0 +1,264 @@
+// ts_api.cu -- the C ABI of libts (include/ts.h): validation, plan-owned scratch, pass
+// scheduling.  All arithmetic is in ts_fused.cu / ts_generic.cu.
+#include <math.h>
+#include <string.h>
+
+#include <new>
+
+#include "ts_internal.h"
+
+namespace ts {
+
+static thread_local std::string g_last_error;
+
+void set_error(const std::string& msg) { g_last_error = msg; }
+
+int cuda_fail(cudaError_t e, const char* what) {
+    g_last_error = std::string("CUDA error: ") + cudaGetErrorString(e) + " in " + what;
+    return TS_ECUDA;
+}
+
+}  // namespace ts
+
+struct ts_plan {
+    ts::LatticeDesc L;
+    int device;
+    size_t elem;              // bytes per element
+    // scratch state buffer for the double-buffered fused passes
+    void* scratch_re;
+    void* scratch_im;
+    // norm workspace
+    double* norm_work;
+    // device staging for ts_evolve_host
+    void* host_re;
+    void* host_im;
+    void* host_pot;
+    cudaStream_t own_stream;
+    // options
+    int64_t opt_path, opt_fuse, opt_seg;
+    // info on the last ts_evolve
+    int64_t info_fused, info_fuse, info_passes, info_launches, info_seg;
+};
+
+namespace {
+
+using ts::set_error;
+
+int fail(int code, const char* msg) {
+    set_error(msg);
+    return code;
+}
+
+int check_device(const ts_plan* plan) {
+    int dev = -1;
+    TS_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev != plan->device) return fail(TS_EINVAL, "plan was created on a different CUDA device");
+    return TS_OK;
+}
+
+bool coef_ok(double a, double b) {
+    return isfinite(a) && isfinite(b) && fabs(a * a + b * b - 1.0) <= 1e-6;
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+bool overlap(const void* a, const void* b, size_t bytes) {
+    const uintptr_t x = reinterpret_cast<uintptr_t>(a), y = reinterpret_cast<uintptr_t>(b);
+    return x < y + bytes && y < x + bytes;
+}
+
+int ensure_alloc(void** p, size_t bytes) {
+    if (*p) return TS_OK;
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) {
+        *p = nullptr;
+        (void)cudaGetLastError();
+        set_error(std::string("scratch allocation failed: ") + cudaGetErrorString(e));
+        return TS_EALLOC;
+    }
+    return TS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* ts_last_error(void) { return ts::g_last_error.c_str(); }
+
+ts_plan* ts_plan_create(int64_t nx, int64_t ny, int dtype, int boundary) {
+    if (nx < 1 || ny < 1) { set_error("nx and ny must be >= 1"); return nullptr; }
+    if (nx > (int64_t(1) << 31) || ny > (int64_t(1) << 31) || nx * ny >= (int64_t(1) << 62) / 16) {
+        set_error("lattice too large");
+        return nullptr;
+    }
+    if (dtype != TS_F32 && dtype != TS_F64) { set_error("unknown dtype"); return nullptr; }
+    if (boundary != TS_CLOSED && boundary != TS_PERIODIC) {
+        set_error("unknown boundary");
+        return nullptr;
+    }
+    if (boundary == TS_PERIODIC && (nx % 2 || ny % 2)) {
+        set_error("periodic boundaries need even nx and ny (an odd ring cannot be split into "
+                  "disjoint pairs)");
+        return nullptr;
+    }
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { ts::cuda_fail(e, "cudaGetDevice"); return nullptr; }
+    ts_plan* p = new (std::nothrow) ts_plan();
+    if (!p) { set_error("out of host memory"); return nullptr; }
+    memset(p, 0, sizeof(*p));
+    p->L.nx = nx; p->L.ny = ny; p->L.dtype = dtype; p->L.periodic = boundary == TS_PERIODIC;
+    p->device = dev;
+    p->elem = dtype == TS_F32 ? 4 : 8;
+    return p;
+}
+
+int ts_plan_destroy(ts_plan* plan) {
+    if (!plan) return TS_OK;
+    cudaFree(plan->scratch_re);
+    cudaFree(plan->scratch_im);
+    cudaFree(plan->norm_work);
+    cudaFree(plan->host_re);
+    cudaFree(plan->host_im);
+    cudaFree(plan->host_pot);
+    if (plan->own_stream) cudaStreamDestroy(plan->own_stream);
+    delete plan;
+    return TS_OK;
+}
+
+int ts_plan_set_option(ts_plan* plan, const char* name, int64_t value) {
+    if (!plan || !name) return fail(TS_EINVAL, "NULL plan or option name");
+    if (!strcmp(name, "path")) {
+        if (value < 0 || value > 2) return fail(TS_EINVAL, "path must be 0, 1 or 2");
+        plan->opt_path = value;
+    } else if (!strcmp(name, "fuse_steps")) {
+        if (value < 0 || value > TS_MAX_FUSE) return fail(TS_EINVAL, "fuse_steps out of range");
+        plan->opt_fuse = value;
+    } else if (!strcmp(name, "seg_rows")) {
+        if (value < 0 || value % 2) return fail(TS_EINVAL, "seg_rows must be even and >= 0");
+        plan->opt_seg = value;
+    } else {
+        return fail(TS_EINVAL, "unknown option");
+    }
+    return TS_OK;
+}
+
+int ts_plan_get_info(const ts_plan* plan, const char* name, int64_t* out) {
+    if (!plan || !name || !out) return fail(TS_EINVAL, "NULL argument");
+    if (!strcmp(name, "fused")) *out = plan->info_fused;
+    else if (!strcmp(name, "fuse_steps")) *out = plan->info_fuse;
+    else if (!strcmp(name, "passes")) *out = plan->info_passes;
+    else if (!strcmp(name, "launches")) *out = plan->info_launches;
+    else if (!strcmp(name, "seg_rows")) *out = plan->info_seg;
+    else return fail(TS_EINVAL, "unknown info name");
+    return TS_OK;
+}
+
+int ts_evolve(ts_plan* plan, void* psi_re, void* psi_im, double a_half, double b_half,
+              double a_full, double b_full, const void* pot, int64_t n_steps, void* cuda_stream) {
+    if (!plan) return fail(TS_EINVAL, "NULL plan");
+    if (!psi_re || !psi_im) return fail(TS_EINVAL, "NULL psi plane");
+    if (n_steps < 0) return fail(TS_EINVAL, "n_steps < 0");
+    if (!coef_ok(a_half, b_half) || !coef_ok(a_full, b_full))
+        return fail(TS_EINVAL, "coefficients must be finite with |a^2 + b^2 - 1| <= 1e-6");
+    const ts::LatticeDesc& L = plan->L;
+    const size_t plane_bytes = (size_t)L.nx * (size_t)L.ny * plan->elem;
+    if (!aligned16(psi_re) || !aligned16(psi_im) || (pot && !aligned16(pot)))
+        return fail(TS_EINVAL, "device pointers must be 16-byte aligned");
+    if (overlap(psi_re, psi_im, plane_bytes)) return fail(TS_EINVAL, "psi_re and psi_im overlap");
+    if (pot && (overlap(pot, psi_re, plane_bytes) || overlap(pot, psi_im, plane_bytes) ||
+                overlap((const char*)pot + plane_bytes, psi_re, plane_bytes) ||
+                overlap((const char*)pot + plane_bytes, psi_im, plane_bytes)))
+        return fail(TS_EINVAL, "pot_phase overlaps psi");
+    int rc = check_device(plan);
+    if (rc != TS_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+
+    plan->info_fused = plan->info_fuse = plan->info_passes = plan->info_launches = 0;
+    plan->info_seg = 0;
+    if (n_steps == 0) return TS_OK;
+
+    const ts::StepCoef c{a_half, b_half, a_full, b_full};
+    const bool can_fuse = ts::fused_supported(L, c);
+    if (plan->opt_path == 2 && !can_fuse)
+        return fail(TS_EUNSUPPORTED,
+                    "fused kernel needs nx % 4 == 0, even ny and cos(theta) > 0.25");
+    if (plan->opt_path == 1 || !can_fuse)
+        return ts::generic_evolve(L, psi_re, psi_im, c, pot, n_steps, st, &plan->info_launches);
+
+    rc = ensure_alloc(&plan->scratch_re, plane_bytes);
+    if (rc == TS_OK) rc = ensure_alloc(&plan->scratch_im, plane_bytes);
+    if (rc != TS_OK) return rc;
+
+    const int S = plan->opt_fuse ? (int)plan->opt_fuse : ts::fused_default_steps(L, pot != nullptr);
+    const int seg = plan->opt_seg ? (int)plan->opt_seg : ts::fused_default_seg_rows(L, S);
+    void* cur_re = psi_re; void* cur_im = psi_im;
+    void* nxt_re = plan->scratch_re; void* nxt_im = plan->scratch_im;
+    int64_t left = n_steps;
+    while (left > 0) {
+        const int s = left >= S ? S : (int)left;
+        rc = ts::fused_pass(L, cur_re, cur_im, nxt_re, nxt_im, c, pot, s, seg, st);
+        if (rc != TS_OK) return rc;
+        void* t;
+        t = cur_re; cur_re = nxt_re; nxt_re = t;
+        t = cur_im; cur_im = nxt_im; nxt_im = t;
+        left -= s;
+        ++plan->info_passes;
+        ++plan->info_launches;
+    }
+    if (cur_re != psi_re) {   // odd number of passes: the result sits in the scratch buffer
+        TS_CUDA_TRY(cudaMemcpyAsync(psi_re, cur_re, plane_bytes, cudaMemcpyDeviceToDevice, st));
+        TS_CUDA_TRY(cudaMemcpyAsync(psi_im, cur_im, plane_bytes, cudaMemcpyDeviceToDevice, st));
+        plan->info_launches += 2;
+    }
+    plan->info_fused = 1;
+    plan->info_fuse = S;
+    plan->info_seg = seg;
+    return TS_OK;
+}
+
+int ts_norm(ts_plan* plan, const void* psi_re, const void* psi_im, double* out, void* cuda_stream) {
+    if (!plan) return fail(TS_EINVAL, "NULL plan");
+    if (!psi_re || !psi_im || !out) return fail(TS_EINVAL, "NULL argument");
+    int rc = check_device(plan);
+    if (rc != TS_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    rc = ensure_alloc(reinterpret_cast<void**>(&plan->norm_work),
+                      ts::norm_workspace_doubles() * sizeof(double));
+    if (rc != TS_OK) return rc;
+    rc = ts::norm2_device(plan->L, psi_re, psi_im, plan->norm_work, st);
+    if (rc != TS_OK) return rc;
+    TS_CUDA_TRY(cudaMemcpyAsync(out, plan->norm_work, sizeof(double), cudaMemcpyDeviceToHost, st));
+    TS_CUDA_TRY(cudaStreamSynchronize(st));
+    return TS_OK;
+}
+
+int ts_evolve_host(ts_plan* plan, void* re_h, void* im_h, double a_half, double b_half,
+                   double a_full, double b_full, const void* pot_h, int64_t n_steps) {
+    if (!plan) return fail(TS_EINVAL, "NULL plan");
+    if (!re_h || !im_h) return fail(TS_EINVAL, "NULL psi plane");
+    int rc = check_device(plan);
+    if (rc != TS_OK) return rc;
+    const size_t plane_bytes = (size_t)plan->L.nx * (size_t)plan->L.ny * plan->elem;
+    rc = ensure_alloc(&plan->host_re, plane_bytes);
+    if (rc == TS_OK) rc = ensure_alloc(&plan->host_im, plane_bytes);
+    if (rc == TS_OK && pot_h) rc = ensure_alloc(&plan->host_pot, 2 * plane_bytes);
+    if (rc != TS_OK) return rc;
+    if (!plan->own_stream)
+        TS_CUDA_TRY(cudaStreamCreateWithFlags(&plan->own_stream, cudaStreamNonBlocking));
+    cudaStream_t st = plan->own_stream;
+    TS_CUDA_TRY(cudaMemcpyAsync(plan->host_re, re_h, plane_bytes, cudaMemcpyHostToDevice, st));
+    TS_CUDA_TRY(cudaMemcpyAsync(plan->host_im, im_h, plane_bytes, cudaMemcpyHostToDevice, st));
+    if (pot_h)
+        TS_CUDA_TRY(cudaMemcpyAsync(plan->host_pot, pot_h, 2 * plane_bytes,
+                                    cudaMemcpyHostToDevice, st));
+    rc = ts_evolve(plan, plan->host_re, plan->host_im, a_half, b_half, a_full, b_full,
+                   pot_h ? plan->host_pot : nullptr, n_steps, st);
+    if (rc != TS_OK) return rc;
+    TS_CUDA_TRY(cudaMemcpyAsync(re_h, plan->host_re, plane_bytes, cudaMemcpyDeviceToHost, st));
+    TS_CUDA_TRY(cudaMemcpyAsync(im_h, plan->host_im, plane_bytes, cudaMemcpyDeviceToHost, st));
+    TS_CUDA_TRY(cudaStreamSynchronize(st));
+    return TS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,50 @@
+// ts_internal.h -- declarations shared by the translation units of libts (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+
+#include "ts.h"
+
+namespace ts {
+
+void set_error(const std::string& msg);
+int cuda_fail(cudaError_t e, const char* what);   // records the CUDA string, returns TS_ECUDA
+
+#define TS_CUDA_TRY(expr)                                             \
+    do {                                                              \
+        cudaError_t e_ = (expr);                                      \
+        if (e_ != cudaSuccess) return ::ts::cuda_fail(e_, #expr);     \
+    } while (0)
+
+// Double-precision description of one step; each path converts to its own arithmetic form.
+struct StepCoef {
+    double a_h, b_h, a_f, b_f;
+};
+
+struct LatticeDesc {
+    int64_t nx, ny;
+    int dtype;      // TS_F32 / TS_F64
+    int periodic;   // 0 closed, 1 periodic
+};
+
+// ---- generic per-sweep path (ts_generic.cu): in place, any nx, ny ------------------------------
+// n_steps full second-order steps, 7 (pot == nullptr) or 9 launches per step.
+int generic_evolve(const LatticeDesc& L, void* re, void* im, const StepCoef& c,
+                   const void* pot, int64_t n_steps, cudaStream_t st, int64_t* launches);
+
+// sum re^2 + im^2 in double -> *d_out (device double).  workspace: >= norm_workspace_doubles().
+int norm2_device(const LatticeDesc& L, const void* re, const void* im, double* d_work,
+                 cudaStream_t st);
+size_t norm_workspace_doubles();
+
+// ---- fused streaming path (ts_fused.cu): out of place, S steps per pass ------------------------
+bool fused_supported(const LatticeDesc& L, const StepCoef& c);
+// One pass: dst <- U2^S src.  S in 1..TS_MAX_FUSE.  seg_rows even, > 0.
+int fused_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
+               void* dst_im, const StepCoef& c, const void* pot, int S, int seg_rows,
+               cudaStream_t st);
+int fused_default_seg_rows(const LatticeDesc& L, int S);
+int fused_default_steps(const LatticeDesc& L, bool pot);
+
+}  // namespace ts
