@@ -173,3 +173,84 @@ def full_pot(cfg: Config, chunk_rows: int = 1024):
         pot[0, y0:y0 + len(ys)] = pr
         pot[1, y0:y0 + len(ys)] = pi
     return pot
+
+
+# ---- the same generators with torch ops (any device), bit-identical to the numpy ones ------------
+def _i64(v: int) -> int:
+    """two's-complement int64 view of a uint64 constant"""
+    v &= 0xFFFFFFFFFFFFFFFF
+    return v - (1 << 64) if v >= (1 << 63) else v
+
+
+def _lsr(z, k: int):
+    """logical shift right of int64 tensors"""
+    return (z >> k) & ((1 << (64 - k)) - 1)
+
+
+def _splitmix64_t(z):
+    z = z + _i64(0x9E3779B97F4A7C15)
+    z = (z ^ _lsr(z, 30)) * _i64(0xBF58476D1CE4E5B9)
+    z = (z ^ _lsr(z, 27)) * _i64(0x94D049BB133111EB)
+    return z ^ _lsr(z, 31)
+
+
+def uniform_pm1_t(seed: int, plane: int, index):
+    """torch twin of uniform_pm1: index is an int64 tensor; returns float64 on its device."""
+    import torch
+    with np.errstate(over="ignore"):
+        key = int(_splitmix64(np.asarray([seed * 2 + plane], dtype=np.uint64))[0])
+    bits = _splitmix64_t(index ^ _i64(key))
+    return _lsr(bits, 11).to(torch.float64) * (2.0 / 9007199254740992.0) - 1.0
+
+
+def _raw_state_t(cfg: Config, y0: int, y1: int, device):
+    import torch
+    ys = torch.arange(y0, y1, dtype=torch.int64, device=device)
+    xs = torch.arange(cfg.nx, dtype=torch.int64, device=device)
+    if cfg.state == "gaussian":
+        X = xs[None, :].to(torch.float64)
+        Y = ys[:, None].to(torch.float64)
+        env = torch.exp(-((X - cfg.x0) ** 2 + (Y - cfg.y0) ** 2) / (4.0 * cfg.sigma ** 2))
+        ph = cfg.kx * X + cfg.ky * Y
+        return env * torch.cos(ph), env * torch.sin(ph)
+    idx = ys[:, None] * cfg.nx + xs[None, :]
+    return uniform_pm1_t(SEED, 0, idx), uniform_pm1_t(SEED, 1, idx)
+
+
+def device_state(cfg: Config, device, chunk_rows: int = 2048):
+    """(re, im, norm2_raw) as torch tensors of the config dtype on `device`; generated in float64
+    chunk by chunk, normalised by the float64 raw norm, then cast (same recipe as full_state).
+    For random states the values are bit-identical to the numpy path given the same norm2."""
+    import torch
+    dt = torch.float32 if cfg.dtype == "f32" else torch.float64
+    parts = []
+    for y0 in range(0, cfg.ny, chunk_rows):
+        r, i = _raw_state_t(cfg, y0, min(cfg.ny, y0 + chunk_rows), device)
+        parts.append(float(torch.sum(r * r + i * i, dtype=torch.float64)))
+    n2 = math.fsum(parts)
+    s = 1.0 / math.sqrt(n2)
+    re = torch.empty((cfg.ny, cfg.nx), dtype=dt, device=device)
+    im = torch.empty((cfg.ny, cfg.nx), dtype=dt, device=device)
+    for y0 in range(0, cfg.ny, chunk_rows):
+        y1 = min(cfg.ny, y0 + chunk_rows)
+        r, i = _raw_state_t(cfg, y0, y1, device)
+        re[y0:y1] = (r * s).to(dt)
+        im[y0:y1] = (i * s).to(dt)
+    return re, im, n2
+
+
+def device_pot(cfg: Config, device, chunk_rows: int = 2048):
+    """pot_phase [2][ny][nx] of the config dtype on `device` (float64 cos/sin, then cast)."""
+    import torch
+    if not cfg.has_pot:
+        return None
+    dt = torch.float32 if cfg.dtype == "f32" else torch.float64
+    pot = torch.empty((2, cfg.ny, cfg.nx), dtype=dt, device=device)
+    X = torch.arange(cfg.nx, dtype=torch.float64, device=device)[None, :]
+    for y0 in range(0, cfg.ny, chunk_rows):
+        y1 = min(cfg.ny, y0 + chunk_rows)
+        Y = torch.arange(y0, y1, dtype=torch.float64, device=device)[:, None]
+        V = 0.5 * cfg.omega ** 2 * ((X - cfg.cx) ** 2 + (Y - cfg.cy) ** 2)
+        pot[0, y0:y1] = torch.cos(V).to(dt)
+        pot[1, y0:y1] = (-torch.sin(V)).to(dt)
+    return pot
