@@ -13,8 +13,8 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 INCLUDE = PKG.parent / "include"
 LIB = PKG / "libts.so"
-SOURCES = ["ts_api.cu", "ts_generic.cu", "ts_fused.cu"]
-HEADERS = [CSRC / "ts_internal.h", INCLUDE / "ts.h"]
+SOURCES = ["ts_api.cu", "ts_generic.cu", "ts_fused.cu", "ts_stream.cu"]
+HEADERS = [CSRC / "ts_internal.h", CSRC / "ts_rows.cuh", INCLUDE / "ts.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]
 

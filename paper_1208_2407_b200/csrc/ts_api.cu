@@ -35,9 +35,9 @@ struct ts_plan {
     void* host_pot;
     cudaStream_t own_stream;
     // options
-    int64_t opt_path, opt_fuse, opt_seg;
+    int64_t opt_path, opt_fuse, opt_seg, opt_variant, opt_slots;
     // info on the last ts_evolve
-    int64_t info_fused, info_fuse, info_passes, info_launches, info_seg;
+    int64_t info_fused, info_fuse, info_passes, info_launches, info_seg, info_variant;
 };
 
 namespace {
@@ -137,6 +137,12 @@ int ts_plan_set_option(ts_plan* plan, const char* name, int64_t value) {
     } else if (!strcmp(name, "seg_rows")) {
         if (value < 0 || value % 2) return fail(TS_EINVAL, "seg_rows must be even and >= 0");
         plan->opt_seg = value;
+    } else if (!strcmp(name, "variant")) {
+        if (value < 0 || value > 2) return fail(TS_EINVAL, "variant must be 0, 1 or 2");
+        plan->opt_variant = value;
+    } else if (!strcmp(name, "ring_slots")) {
+        if (value < 0 || value > 64) return fail(TS_EINVAL, "ring_slots out of range");
+        plan->opt_slots = value;
     } else {
         return fail(TS_EINVAL, "unknown option");
     }
@@ -150,6 +156,7 @@ int ts_plan_get_info(const ts_plan* plan, const char* name, int64_t* out) {
     else if (!strcmp(name, "passes")) *out = plan->info_passes;
     else if (!strcmp(name, "launches")) *out = plan->info_launches;
     else if (!strcmp(name, "seg_rows")) *out = plan->info_seg;
+    else if (!strcmp(name, "variant")) *out = plan->info_variant;
     else return fail(TS_EINVAL, "unknown info name");
     return TS_OK;
 }
@@ -175,7 +182,7 @@ int ts_evolve(ts_plan* plan, void* psi_re, void* psi_im, double a_half, double b
     cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
 
     plan->info_fused = plan->info_fuse = plan->info_passes = plan->info_launches = 0;
-    plan->info_seg = 0;
+    plan->info_seg = plan->info_variant = 0;
     if (n_steps == 0) return TS_OK;
 
     const ts::StepCoef c{a_half, b_half, a_full, b_full};
@@ -192,12 +199,21 @@ int ts_evolve(ts_plan* plan, void* psi_re, void* psi_im, double a_half, double b
 
     const int S = plan->opt_fuse ? (int)plan->opt_fuse : ts::fused_default_steps(L, pot != nullptr);
     const int seg = plan->opt_seg ? (int)plan->opt_seg : ts::fused_default_seg_rows(L, S);
+    const bool can_stream = ts::stream_supported(L, c);
+    if (plan->opt_variant == 2 && !can_stream)
+        return fail(TS_EUNSUPPORTED, "the TMA ring kernel needs nx >= 128");
+    const bool use_stream = can_stream && plan->opt_variant != 1;
+    plan->info_variant = use_stream ? 2 : 1;
     void* cur_re = psi_re; void* cur_im = psi_im;
     void* nxt_re = plan->scratch_re; void* nxt_im = plan->scratch_im;
     int64_t left = n_steps;
     while (left > 0) {
         const int s = left >= S ? S : (int)left;
-        rc = ts::fused_pass(L, cur_re, cur_im, nxt_re, nxt_im, c, pot, s, seg, st);
+        if (use_stream)
+            rc = ts::stream_pass(L, cur_re, cur_im, nxt_re, nxt_im, c, pot, s, seg,
+                                 (int)plan->opt_slots, st);
+        else
+            rc = ts::fused_pass(L, cur_re, cur_im, nxt_re, nxt_im, c, pot, s, seg, st);
         if (rc != TS_OK) return rc;
         void* t;
         t = cur_re; cur_re = nxt_re; nxt_re = t;

@@ -1,0 +1,129 @@
+// ts_rows.cuh -- per-lane row arithmetic shared by the fused kernels (device code only).
+//
+// A lane owns 4 consecutive sites of a row (re[4], im[4]).  Every pair rotation
+// [[a, i b],[i b, a]] is applied in the scaled form a * [[1, i t],[i t, 1]],
+// t = b/a: two FMAs per site per sweep; the factors a are collected into one multiplication
+// at the store.  At a closed edge the unpaired site is multiplied by 1/a instead, so that the
+// deferred factor stays uniform over the lattice.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ts {
+namespace rows {
+
+constexpr int kStripSites = 128;   // 32 lanes x 4 sites
+
+template <typename T>
+struct Row4 {
+    T re[4];
+    T im[4];
+};
+
+__device__ __forceinline__ void ld4(const float* __restrict__ p, float (&v)[4]) {
+    const float4 q = __ldg(reinterpret_cast<const float4*>(p));
+    v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+}
+__device__ __forceinline__ void ld4(const double* __restrict__ p, double (&v)[4]) {
+    const double2 a = __ldg(reinterpret_cast<const double2*>(p));
+    const double2 b = __ldg(reinterpret_cast<const double2*>(p) + 1);
+    v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+}
+__device__ __forceinline__ void st4(float* __restrict__ p, const float (&v)[4], float s) {
+    *reinterpret_cast<float4*>(p) = make_float4(v[0] * s, v[1] * s, v[2] * s, v[3] * s);
+}
+__device__ __forceinline__ void st4(double* __restrict__ p, const double (&v)[4], double s) {
+    reinterpret_cast<double2*>(p)[0] = make_double2(v[0] * s, v[1] * s);
+    reinterpret_cast<double2*>(p)[1] = make_double2(v[2] * s, v[3] * s);
+}
+
+template <typename T>
+__device__ __forceinline__ void zero_row(Row4<T>& r) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { r.re[i] = T(0); r.im[i] = T(0); }
+}
+
+// scaled pair rotation: (p, q) <- (p + i t q, q + i t p), from the old values of both
+template <typename T>
+__device__ __forceinline__ void rot(T& rp, T& ip, T& rq, T& iq, T t) {
+    const T nrp = fma(-t, iq, rp);
+    const T nip = fma(t, rq, ip);
+    const T nrq = fma(-t, ip, rq);
+    const T niq = fma(t, rp, iq);
+    rp = nrp; ip = nip; rq = nrq; iq = niq;
+}
+
+// X-even sweep on one row: pairs (0,1), (2,3) of the lane's four sites
+template <typename T>
+__device__ __forceinline__ void xe(Row4<T>& r, T t) {
+    rot(r.re[0], r.im[0], r.re[1], r.im[1], t);
+    rot(r.re[2], r.im[2], r.re[3], r.im[3], t);
+}
+
+// per-lane coefficients of the cross-lane X-odd pair; differ from (t, t, 1, 1) only in strips
+// that touch a closed domain edge
+template <typename T>
+struct XEdge {
+    T t_up;   // coupling of my site 0 to the previous lane's site 3
+    T t_dn;   // coupling of my site 3 to the next lane's site 0
+    T c0;     // factor on my site 0 (1/a when it is the unpaired edge site)
+    T c3;     // factor on my site 3
+};
+
+// X-odd sweep on one row: pair (1,2) in-thread, pair (3, 0 of next lane) by shuffle.
+template <typename T, bool EDGE>
+__device__ __forceinline__ void xo(Row4<T>& r, T t, const XEdge<T>& e) {
+    const T up_re = __shfl_up_sync(0xffffffffu, r.re[3], 1);
+    const T up_im = __shfl_up_sync(0xffffffffu, r.im[3], 1);
+    const T dn_re = __shfl_down_sync(0xffffffffu, r.re[0], 1);
+    const T dn_im = __shfl_down_sync(0xffffffffu, r.im[0], 1);
+    rot(r.re[1], r.im[1], r.re[2], r.im[2], t);
+    if (EDGE) {
+        const T r0 = r.re[0] * e.c0, i0 = r.im[0] * e.c0;
+        const T r3 = r.re[3] * e.c3, i3 = r.im[3] * e.c3;
+        r.re[0] = fma(-e.t_up, up_im, r0);
+        r.im[0] = fma(e.t_up, up_re, i0);
+        r.re[3] = fma(-e.t_dn, dn_im, r3);
+        r.im[3] = fma(e.t_dn, dn_re, i3);
+    } else {
+        const T r0 = r.re[0], i0 = r.im[0], r3 = r.re[3], i3 = r.im[3];
+        r.re[0] = fma(-t, up_im, r0);
+        r.im[0] = fma(t, up_re, i0);
+        r.re[3] = fma(-t, dn_im, r3);
+        r.im[3] = fma(t, dn_re, i3);
+    }
+}
+
+// vertical pair sweep between two rows held by the same lane
+template <typename T>
+__device__ __forceinline__ void ypair(Row4<T>& a, Row4<T>& b, T t) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) rot(a.re[i], a.im[i], b.re[i], b.im[i], t);
+}
+
+template <typename T>
+__device__ __forceinline__ void scale_row(Row4<T>& r, T s) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { r.re[i] *= s; r.im[i] *= s; }
+}
+
+// psi <- psi * (pr + i pi) on one row
+template <typename T>
+__device__ __forceinline__ void phase_row(Row4<T>& r, const T (&pr)[4], const T (&pi)[4]) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const T a = r.re[i], b = r.im[i];
+        r.re[i] = fma(-b, pi[i], a * pr[i]);
+        r.im[i] = fma(b, pr[i], a * pi[i]);
+    }
+}
+
+__device__ __forceinline__ int wrap_index(int v, int n) {
+    while (v < 0) v += n;
+    while (v >= n) v -= n;
+    return v;
+}
+
+
+}  // namespace rows
+}  // namespace ts

@@ -1,0 +1,381 @@
+// ts_stream.cu -- fused streaming kernel v2: TMA bulk copies into a per-warp shared-memory ring.
+//
+// Same decomposition and arithmetic as ts_fused.cu (one warp per 128-site column strip and
+// y-segment, 4 sites per lane, S chained steps as a register pipeline over row pairs), but the
+// rows are brought on chip by cp.async.bulk (TMA, completion on an mbarrier) into a ring of NST
+// row-pair slots owned by the warp, several iterations ahead of their use.  Global-load latency
+// is therefore hidden by shared memory, not by registers, which removes the long-scoreboard
+// stalls that bound v1 (profiles/r1a_*): registers only hold the S+1 row pairs of the pipeline.
+// The register pipeline is unrolled over its rotation period S+1 so that rows never move between
+// registers.  Potential-phase rows travel in the same slots and are kept S+1 iterations longer,
+// because stage j of the pipeline applies the phase to rows that arrived j iterations earlier.
+//
+// Results are written straight from registers with 128-bit stores into the other buffer
+// (double buffering); halo columns of a strip are recomputed and discarded
+// (PAPER.md:115).
+#include <math.h>
+
+#include "ts_internal.h"
+#include "ts_rows.cuh"
+
+namespace ts {
+namespace {
+
+using namespace rows;
+
+constexpr int kWarps = 4;
+
+template <typename T>
+struct StreamParams {
+    const T* src_re;
+    const T* src_im;
+    T* dst_re;
+    T* dst_im;
+    const T* pot_re;
+    const T* pot_im;
+    int nx, ny;
+    int n_strips, wi, halo, seg_rows;
+    int nst;        // ring slots per warp
+    T t_h, t_f, sec_h, sec_f, out_scale;
+};
+
+// ---- PTX: mbarrier + bulk async copy (TMA) -------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "WAIT_LOOP:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra WAIT_DONE;\n\t"
+        "bra WAIT_LOOP;\n\t"
+        "WAIT_DONE:\n\t"
+        "}" ::"r"(bar), "r"(parity)
+        : "memory");
+}
+// global -> shared bulk copy; bytes % 16 == 0, both addresses 16-byte aligned
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes,
+                                         uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+        ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
+        : "memory");
+}
+
+__device__ __forceinline__ void lds4(uint32_t addr, float (&v)[4]) {
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]) : "r"(addr));
+}
+__device__ __forceinline__ void lds4(uint32_t addr, double (&v)[4]) {
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[0]), "=d"(v[1]) : "r"(addr));
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[2]), "=d"(v[3]) : "r"(addr + 16));
+}
+
+template <typename T>
+struct StreamCtx {
+    int xl;          // lane's first column (unwrapped; may lie outside the lattice)
+    bool xvalid;     // lane's sites exist (always when periodic)
+    bool xedge;      // warp-uniform: strip touches a closed edge in x
+    XEdge<T> e;
+    uint32_t ring;   // shared address of the warp's slot ring
+    uint32_t lane_off;   // byte offset of the lane's 4 sites inside a row chunk
+};
+
+// One second-order step of the register pipeline (see ts_fused.cu::step_stage for the roles).
+//   in : (a0, a1) = rows (yj, yj+1) before the step; (g, h) = rows (yj-2, yj-1) in mid-step state
+//   out: (g, h) = rows (yj-2, yj-1) after the step; (a0, a1) = rows (yj, yj+1) in mid-step state
+// pot0 / pot1: shared addresses of the potential rows yj (row 0 of its slot) and yj-1 (row 1 of
+// the previous slot), valid when POT.
+template <typename T, bool POT, bool PER>
+__device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const StreamCtx<T>& c,
+                                             int yj, Row4<T>& a0, Row4<T>& a1, Row4<T>& g,
+                                             Row4<T>& h, uint32_t pot_yj, uint32_t pot_yjm1) {
+    constexpr uint32_t ROWB = kStripSites * sizeof(T);
+    xe(a0, p.t_h); xe(a1, p.t_h);
+    if (c.xedge) { xo<T, true>(a0, p.t_h, c.e); xo<T, true>(a1, p.t_h, c.e); }
+    else { xo<T, false>(a0, p.t_h, c.e); xo<T, false>(a1, p.t_h, c.e); }
+    ypair(a0, a1, p.t_h);
+    const bool yedge = !PER && (yj == 0 || yj == p.ny);
+    if (!POT) {
+        if (yedge) { if (yj == 0) scale_row(a0, p.sec_f); else scale_row(h, p.sec_f); }
+        else ypair(h, a0, p.t_f);
+    } else {
+        if (yedge) {
+            if (yj == 0) scale_row(a0, p.sec_h * p.sec_h); else scale_row(h, p.sec_h * p.sec_h);
+        } else {
+            ypair(h, a0, p.t_h);
+        }
+        const bool lo_ok = c.xvalid && (PER || (yj - 1 >= 0 && yj - 1 < p.ny));
+        const bool hi_ok = c.xvalid && (PER || (yj >= 0 && yj < p.ny));
+        if (lo_ok) {
+            T pr[4], pi[4];
+            lds4(pot_yjm1 + c.lane_off, pr);
+            lds4(pot_yjm1 + ROWB + c.lane_off, pi);
+            phase_row(h, pr, pi);
+        }
+        if (hi_ok) {
+            T pr[4], pi[4];
+            lds4(pot_yj + c.lane_off, pr);
+            lds4(pot_yj + ROWB + c.lane_off, pi);
+            phase_row(a0, pr, pi);
+        }
+        if (!yedge) ypair(h, a0, p.t_h);
+    }
+    ypair(g, h, p.t_h);
+    if (c.xedge) { xo<T, true>(g, p.t_h, c.e); xo<T, true>(h, p.t_h, c.e); }
+    else { xo<T, false>(g, p.t_h, c.e); xo<T, false>(h, p.t_h, c.e); }
+    xe(g, p.t_h); xe(h, p.t_h);
+}
+
+template <typename T, int S, bool POT, bool PER>
+__global__ void __launch_bounds__(kWarps * 32)
+stream_kernel(const StreamParams<T> p) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    constexpr int P = S + 1;                  // register slots = rotation period of the pipeline
+    constexpr int R = POT ? S + 1 : 1;        // iterations a ring slot stays live after its arrival
+    constexpr uint32_t ROWB = kStripSites * sizeof(T);
+    constexpr int NROW = POT ? 8 : 4;         // re0 im0 re1 im1 [pr0 pi0 pr1 pi1]
+    constexpr uint32_t SLOTB = NROW * ROWB;
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const int strip = blockIdx.x * kWarps + warp;
+    if (strip >= p.n_strips) return;
+    const int NST = p.nst;
+    const int DIST = NST - R;                 // prefetch distance in iterations
+
+    const int x0 = strip * p.wi;
+    const int xs = x0 - p.halo;               // first column of the strip window
+    const int xb = xs + 4 * lane;
+    StreamCtx<T> c;
+    c.xl = xb;
+    c.xvalid = PER ? true : (xb >= 0 && xb < p.nx);
+    c.xedge = !PER && (xs < 0 || xs + kStripSites > p.nx);
+    c.e.t_up = (xb == 0 || xb == p.nx) ? T(0) : p.t_h;
+    c.e.t_dn = (xb + 4 == p.nx || xb + 4 == 0) ? T(0) : p.t_h;
+    c.e.c0 = (xb == 0) ? p.sec_h : T(1);
+    c.e.c3 = (xb + 4 == p.nx) ? p.sec_h : T(1);
+    c.ring = smem_u32(smem_raw) + warp * NST * SLOTB;
+    c.lane_off = lane * 4 * sizeof(T);
+    const uint32_t bars = smem_u32(smem_raw) + kWarps * NST * SLOTB + warp * NST * 8;
+    const bool store_ok = (4 * lane >= p.halo) && (4 * lane < kStripSites - p.halo) && (xb < p.nx);
+
+    // the strip window [xs, xs+128) as at most two contiguous global pieces (warp-uniform)
+    int gx_a, off_a, len_a, len_b;            // piece B always starts at global column 0
+    if (PER) {
+        gx_a = wrap_index(xs, p.nx);
+        off_a = 0;
+        len_a = min(kStripSites, p.nx - gx_a);
+        len_b = kStripSites - len_a;
+    } else {
+        gx_a = max(xs, 0);
+        off_a = gx_a - xs;
+        len_a = min(xs + kStripSites, p.nx) - gx_a;
+        len_b = 0;
+    }
+    const uint32_t slot_tx = NROW * (len_a + len_b) * sizeof(T);
+
+    // lane r < NROW issues the copies of row r of a slot
+    const T* my_plane = nullptr;
+    if (lane < NROW) {
+        const int plane = lane & 1, is_pot = lane >> 2;
+        my_plane = is_pot ? (plane ? p.pot_im : p.pot_re) : (plane ? p.src_im : p.src_re);
+    }
+    const int my_rowsel = (lane >> 1) & 1;
+
+    const int y_out0 = blockIdx.y * p.seg_rows;
+    const int y_out1 = min(y_out0 + p.seg_rows, p.ny);
+    const int y_in0 = y_out0 - 2 * S;
+    const int n_iter = (y_out1 - y_out0) / 2 + 2 * S;
+
+    if (lane == 0) {
+        for (int s = 0; s < NST; ++s) mbar_init(bars + 8 * s, 1);
+        mbar_fence_init();
+    }
+    __syncwarp();
+
+    // fetch the rows of iteration k into ring slot `slot`
+    auto issue = [&](int k, int slot) {
+        const int y = y_in0 + 2 * k;
+        const bool rowok = PER ? true : (y >= 0 && y < p.ny);
+        const int yl = PER ? wrap_index(y, p.ny) : y;
+        const uint32_t bar = bars + 8 * slot;
+        if (lane == 0) {
+            if (rowok) mbar_arrive_expect_tx(bar, slot_tx);
+            else mbar_arrive(bar);
+        }
+        __syncwarp();
+        if (rowok && lane < NROW) {
+            const T* src = my_plane + (int64_t)(yl + my_rowsel) * p.nx;
+            const uint32_t dst = c.ring + slot * SLOTB + lane * ROWB;
+            bulk_g2s(dst + off_a * sizeof(T), src + gx_a, len_a * sizeof(T), bar);
+            if (len_b > 0) bulk_g2s(dst + len_a * sizeof(T), src, len_b * sizeof(T), bar);
+        }
+    };
+
+    for (int k = 0; k < DIST; ++k)
+        if (k < n_iter) issue(k, k);
+
+    Row4<T> reg[P][2];
+#pragma unroll
+    for (int s = 0; s < P; ++s) { zero_row(reg[s][0]); zero_row(reg[s][1]); }
+
+    int cs = 0;                 // ring slot of the current iteration
+    uint32_t cph = 0;           // its mbarrier phase parity
+    int rs = DIST % NST;        // ring slot refilled at the top of the current iteration
+
+#pragma unroll 1
+    for (int it0 = 0; it0 < n_iter; it0 += P) {
+#pragma unroll
+        for (int u = 0; u < P; ++u) {
+            const int it = it0 + u;
+            if (it < n_iter) {
+                __syncwarp();
+                if (it + DIST < n_iter) issue(it + DIST, rs);
+                mbar_wait(bars + 8 * cs, cph);
+                const int y = y_in0 + 2 * it;
+                const bool rowok = PER ? true : (y >= 0 && y < p.ny);
+                Row4<T>& a0 = reg[u][0];
+                Row4<T>& a1 = reg[u][1];
+                if (rowok && c.xvalid) {
+                    const uint32_t base = c.ring + cs * SLOTB + c.lane_off;
+                    lds4(base, a0.re);
+                    lds4(base + ROWB, a0.im);
+                    lds4(base + 2 * ROWB, a1.re);
+                    lds4(base + 3 * ROWB, a1.im);
+                } else {
+                    zero_row(a0);
+                    zero_row(a1);
+                }
+#pragma unroll
+                for (int j = 0; j < S; ++j) {
+                    uint32_t pot_yj = 0, pot_yjm1 = 0;
+                    if (POT) {
+                        int s0 = cs - j;      if (s0 < 0) s0 += NST;
+                        int s1 = s0 - 1;      if (s1 < 0) s1 += NST;
+                        pot_yj = c.ring + s0 * SLOTB + 4 * ROWB;
+                        pot_yjm1 = c.ring + s1 * SLOTB + 6 * ROWB;
+                    }
+                    stream_stage<T, POT, PER>(p, c, y - 2 * j, reg[(u - j + P) % P][0],
+                                              reg[(u - j + P) % P][1],
+                                              reg[(u - j - 1 + 2 * P) % P][0],
+                                              reg[(u - j - 1 + 2 * P) % P][1], pot_yj, pot_yjm1);
+                }
+                if (it >= 2 * S && store_ok) {
+                    const Row4<T>& o0 = reg[(u - S + 2 * P) % P][0];
+                    const Row4<T>& o1 = reg[(u - S + 2 * P) % P][1];
+                    const int64_t off = (int64_t)(y - 2 * S) * p.nx + xb;
+                    st4(p.dst_re + off, o0.re, p.out_scale);
+                    st4(p.dst_im + off, o0.im, p.out_scale);
+                    st4(p.dst_re + off + p.nx, o1.re, p.out_scale);
+                    st4(p.dst_im + off + p.nx, o1.im, p.out_scale);
+                }
+                if (++cs == NST) { cs = 0; cph ^= 1; }
+                if (++rs == NST) rs = 0;
+            }
+        }
+    }
+}
+
+template <typename T, int S, bool POT, bool PER>
+int launch(const StreamParams<T>& p, cudaStream_t st) {
+    constexpr uint32_t SLOTB = (POT ? 8 : 4) * kStripSites * sizeof(T);
+    const size_t smem = (size_t)kWarps * p.nst * (SLOTB + 8);
+    auto kern = stream_kernel<T, S, POT, PER>;
+    static size_t configured = 0;    // per instantiation
+    if (smem > configured) {
+        TS_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem));
+        configured = smem;
+    }
+    const int n_seg = (p.ny + p.seg_rows - 1) / p.seg_rows;
+    dim3 grid((p.n_strips + kWarps - 1) / kWarps, n_seg);
+    kern<<<grid, kWarps * 32, smem, st>>>(p);
+    TS_CUDA_TRY(cudaGetLastError());
+    return TS_OK;
+}
+
+template <typename T, int S>
+int launch_s(const StreamParams<T>& p, bool pot, bool per, cudaStream_t st) {
+    if (pot) return per ? launch<T, S, true, true>(p, st) : launch<T, S, true, false>(p, st);
+    return per ? launch<T, S, false, true>(p, st) : launch<T, S, false, false>(p, st);
+}
+
+template <typename T>
+int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T* dst_im,
+           const StepCoef& c, const T* pot, int S, int seg_rows, int nst, cudaStream_t st) {
+    StreamParams<T> p;
+    p.src_re = src_re; p.src_im = src_im; p.dst_re = dst_re; p.dst_im = dst_im;
+    p.pot_re = pot;
+    p.pot_im = pot ? pot + L.nx * L.ny : nullptr;
+    p.nx = (int)L.nx; p.ny = (int)L.ny;
+    p.halo = (2 * S + 3) / 4 * 4;
+    p.wi = kStripSites - 2 * p.halo;
+    p.n_strips = (int)((L.nx + p.wi - 1) / p.wi);
+    p.seg_rows = seg_rows;
+    const int live = pot ? S + 1 : 1;
+    if (nst <= 0) nst = stream_default_slots(L, S, pot != nullptr);
+    if (nst < live + 1) nst = live + 1;
+    const size_t slotb = (size_t)(pot ? 8 : 4) * kStripSites * sizeof(T);
+    while (nst > live + 1 && (size_t)kWarps * nst * (slotb + 8) > 227u * 1024u) --nst;
+    p.nst = nst;
+    p.t_h = (T)(c.b_h / c.a_h);
+    p.t_f = (T)(c.b_f / c.a_f);
+    p.sec_h = (T)(1.0 / c.a_h);
+    p.sec_f = (T)(1.0 / c.a_f);
+    const double per_step = pot ? pow(c.a_h, 8) : pow(c.a_h, 6) * c.a_f;
+    p.out_scale = (T)pow(per_step, S);
+    const bool per = L.periodic != 0;
+    switch (S) {
+        case 1: return launch_s<T, 1>(p, pot != nullptr, per, st);
+        case 2: return launch_s<T, 2>(p, pot != nullptr, per, st);
+        case 3: return launch_s<T, 3>(p, pot != nullptr, per, st);
+        case 4: return launch_s<T, 4>(p, pot != nullptr, per, st);
+    }
+    set_error("stream_pass: steps per pass out of range");
+    return TS_EINVAL;
+}
+
+}  // namespace
+
+bool stream_supported(const LatticeDesc& L, const StepCoef& c) {
+    // the strip window must split into at most two contiguous pieces of a row
+    return fused_supported(L, c) && L.nx >= kStripSites;
+}
+
+int stream_default_slots(const LatticeDesc& L, int S, bool pot) {
+    // sized so that 2-4 blocks of 4 warps fit the 227 KB of an SM with >= 3 iterations in flight
+    if (L.dtype == TS_F32) return pot ? S + 4 : 6;
+    return pot ? S + 4 : 6;
+}
+
+int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
+                void* dst_im, const StepCoef& c, const void* pot, int S, int seg_rows, int nst,
+                cudaStream_t st) {
+    if (seg_rows <= 0 || seg_rows % 2) {
+        set_error("stream_pass: seg_rows must be positive and even");
+        return TS_EINVAL;
+    }
+    if (L.dtype == TS_F32)
+        return pass_t<float>(L, (const float*)src_re, (const float*)src_im, (float*)dst_re,
+                             (float*)dst_im, c, (const float*)pot, S, seg_rows, nst, st);
+    return pass_t<double>(L, (const double*)src_re, (const double*)src_im, (double*)dst_re,
+                          (double*)dst_im, c, (const double*)pot, S, seg_rows, nst, st);
+}
+
+}  // namespace ts

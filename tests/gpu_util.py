@@ -14,7 +14,7 @@ def torch_dtype(cfg):
 
 
 def gpu_evolve(cfg, re_np, im_np, pot_np=None, n_steps=None, path=0, fuse=0, seg_rows=0,
-               coeffs=None):
+               coeffs=None, variant=0, ring_slots=0):
     """Upload, ts_evolve, download.  Returns (re, im, info dict)."""
     import torch
     from paper_1208_2407_b200.binding import Plan
@@ -23,6 +23,8 @@ def gpu_evolve(cfg, re_np, im_np, pot_np=None, n_steps=None, path=0, fuse=0, seg
     plan.set_option("path", path)
     plan.set_option("fuse_steps", fuse)
     plan.set_option("seg_rows", seg_rows)
+    plan.set_option("variant", variant)
+    plan.set_option("ring_slots", ring_slots)
     re = torch.from_numpy(np.ascontiguousarray(re_np)).to(dev)
     im = torch.from_numpy(np.ascontiguousarray(im_np)).to(dev)
     pot = None if pot_np is None else torch.from_numpy(np.ascontiguousarray(pot_np)).to(dev)
@@ -32,7 +34,8 @@ def gpu_evolve(cfg, re_np, im_np, pot_np=None, n_steps=None, path=0, fuse=0, seg
     plan.evolve(re, im, *c, pot_phase=pot, n_steps=n)
     torch.cuda.synchronize()
     n2_after = plan.norm(re, im)
-    info = {k: plan.info(k) for k in ("fused", "fuse_steps", "passes", "launches", "seg_rows")}
+    info = {k: plan.info(k) for k in ("fused", "fuse_steps", "passes", "launches", "seg_rows",
+                                     "variant")}
     info["norm2_before"], info["norm2_after"] = n2_before, n2_after
     out = re.cpu().numpy(), im.cpu().numpy()
     plan.destroy()

@@ -37,23 +37,30 @@ def check(cfg, re, im, pot, n_steps, **opts):
 @pytest.mark.parametrize("boundary", ["closed", "periodic"])
 @pytest.mark.parametrize("with_pot", [False, True])
 @pytest.mark.parametrize("fuse", [1, 2, 3, 4])
-def test_fused_f32(nx, ny, boundary, with_pot, fuse):
+@pytest.mark.parametrize("variant", [1, 2])
+def test_fused_f32(nx, ny, boundary, with_pot, fuse, variant):
+    # variant 1 = register-prefetch kernel (ts_fused.cu), 2 = TMA ring kernel (ts_stream.cu)
+    if variant == 2 and nx < 128:
+        pytest.skip("the TMA ring kernel needs nx >= 128 (auto falls back to variant 1)")
     cfg = G.make_cfg(nx, ny, "f32", boundary, 0.3, 9)
     re, im, pot = G.random_inputs(nx, ny, "f32", nx * 1000 + ny, with_pot)
-    info = check(cfg, re, im, pot, 9, path=2, fuse=fuse, seg_rows=32)
-    assert info["fused"] == 1 and info["fuse_steps"] == fuse
+    info = check(cfg, re, im, pot, 9, path=2, fuse=fuse, seg_rows=32, variant=variant)
+    assert info["fused"] == 1 and info["fuse_steps"] == fuse and info["variant"] == variant
     assert info["passes"] == math.ceil(9 / fuse)
 
 
-@pytest.mark.parametrize("nx,ny", [(8, 6), (124, 34), (252, 66)])
+@pytest.mark.parametrize("nx,ny", [(8, 6), (124, 34), (128, 40), (252, 66), (380, 130)])
 @pytest.mark.parametrize("boundary", ["closed", "periodic"])
 @pytest.mark.parametrize("with_pot", [False, True])
 @pytest.mark.parametrize("fuse", [1, 2, 3, 4])
-def test_fused_f64(nx, ny, boundary, with_pot, fuse):
+@pytest.mark.parametrize("variant", [1, 2])
+def test_fused_f64(nx, ny, boundary, with_pot, fuse, variant):
+    if variant == 2 and nx < 128:
+        pytest.skip("the TMA ring kernel needs nx >= 128")
     cfg = G.make_cfg(nx, ny, "f64", boundary, 0.3, 9)
     re, im, pot = G.random_inputs(nx, ny, "f64", nx * 1000 + ny + 1, with_pot)
-    info = check(cfg, re, im, pot, 9, path=2, fuse=fuse, seg_rows=16)
-    assert info["fused"] == 1
+    info = check(cfg, re, im, pot, 9, path=2, fuse=fuse, seg_rows=16, variant=variant)
+    assert info["fused"] == 1 and info["variant"] == variant
 
 
 @pytest.mark.parametrize("nx,ny", [(1, 1), (2, 1), (1, 2), (5, 3), (7, 8), (64, 64), (129, 67),
@@ -78,10 +85,20 @@ def test_auto_path_picks_generic_for_unaligned_shapes():
 
 
 @pytest.mark.parametrize("seg_rows", [2, 6, 64, 0])
-def test_segment_sizes(seg_rows):
+@pytest.mark.parametrize("variant", [1, 2])
+def test_segment_sizes(seg_rows, variant):
     cfg = G.make_cfg(256, 100, "f32", "periodic", 0.25, 8)
     re, im, pot = G.random_inputs(256, 100, "f32", 9, True)
-    check(cfg, re, im, pot, 8, path=2, fuse=3, seg_rows=seg_rows)
+    check(cfg, re, im, pot, 8, path=2, fuse=3, seg_rows=seg_rows, variant=variant)
+
+
+@pytest.mark.parametrize("slots", [2, 3, 5, 12, 64])
+@pytest.mark.parametrize("with_pot", [False, True])
+def test_ring_depths(slots, with_pot):
+    # any ring depth (clamped to what the pipeline needs and to 227 KB) gives the same result
+    cfg = G.make_cfg(380, 70, "f32", "closed", 0.25, 6)
+    re, im, pot = G.random_inputs(380, 70, "f32", 19, with_pot)
+    check(cfg, re, im, pot, 6, path=2, fuse=2, seg_rows=32, variant=2, ring_slots=slots)
 
 
 def test_negative_angle_and_reversibility_on_device():
