@@ -86,27 +86,43 @@ __device__ __forceinline__ void lds4(uint32_t addr, double (&v)[4]) {
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[2]), "=d"(v[3]) : "r"(addr + 16));
 }
 
+// one lane per warp, known to the compiler as a single active lane (no per-lane issue loops)
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred P;\n\t"
+        "elect.sync _|P, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, P;\n\t"
+        "}" : "=r"(pred));
+    return pred != 0;
+}
+
 template <typename T>
 struct StreamCtx {
-    int xl;          // lane's first column (unwrapped; may lie outside the lattice)
-    bool xvalid;     // lane's sites exist (always when periodic)
-    bool xedge;      // warp-uniform: strip touches a closed edge in x
+    bool xvalid;         // lane's sites exist (always when periodic)
+    bool xedge;          // warp-uniform: strip touches a closed edge in x
     XEdge<T> e;
-    uint32_t ring;   // shared address of the warp's slot ring
+    uint32_t ring;       // shared address of the warp's slot ring
     uint32_t lane_off;   // byte offset of the lane's 4 sites inside a row chunk
 };
 
-// One second-order step of the register pipeline (see ts_fused.cu::step_stage for the roles).
+// One second-order step of the register pipeline.
 //   in : (a0, a1) = rows (yj, yj+1) before the step; (g, h) = rows (yj-2, yj-1) in mid-step state
 //   out: (g, h) = rows (yj-2, yj-1) after the step; (a0, a1) = rows (yj, yj+1) in mid-step state
-// pot0 / pot1: shared addresses of the potential rows yj (row 0 of its slot) and yj-1 (row 1 of
-// the previous slot), valid when POT.
-template <typename T, bool POT, bool PER>
+// FIRST / LAST: first / last step of the pass.  Between two chained steps the closing X-even
+// half sweep of one and the opening X-even half sweep of the next act on the same rows back to
+// back, Xe(h) Xe(h) = Xe(f), so an inner boundary applies ONE full-angle X-even sweep at the
+// start of the later step (the deferred cos factor is adjusted in out_scale).
+// pot_yj / pot_yjm1: shared addresses of the potential rows yj (row 0 of its slot) and yj-1
+// (row 1 of the previous slot), valid when POT.
+template <typename T, bool POT, bool PER, bool FIRST, bool LAST>
 __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const StreamCtx<T>& c,
                                              int yj, Row4<T>& a0, Row4<T>& a1, Row4<T>& g,
                                              Row4<T>& h, uint32_t pot_yj, uint32_t pot_yjm1) {
     constexpr uint32_t ROWB = kStripSites * sizeof(T);
-    xe(a0, p.t_h); xe(a1, p.t_h);
+    const T t_open = FIRST ? p.t_h : p.t_f;
+    xe(a0, t_open); xe(a1, t_open);
     if (c.xedge) { xo<T, true>(a0, p.t_h, c.e); xo<T, true>(a1, p.t_h, c.e); }
     else { xo<T, false>(a0, p.t_h, c.e); xo<T, false>(a1, p.t_h, c.e); }
     ypair(a0, a1, p.t_h);
@@ -139,11 +155,36 @@ __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const Str
     ypair(g, h, p.t_h);
     if (c.xedge) { xo<T, true>(g, p.t_h, c.e); xo<T, true>(h, p.t_h, c.e); }
     else { xo<T, false>(g, p.t_h, c.e); xo<T, false>(h, p.t_h, c.e); }
-    xe(g, p.t_h); xe(h, p.t_h);
+    if (LAST) { xe(g, p.t_h); xe(h, p.t_h); }
 }
 
-template <typename T, int S, bool POT, bool PER>
-__global__ void __launch_bounds__(kWarps * 32)
+// The same step WITHOUT a potential, regrouped.  Horizontal sweeps act inside a row and vertical
+// sweeps act along a column with the same scalar coefficients, so every X sweep commutes with every
+// Y sweep (tensor-product structure; pinned on the oracle by test_xy_regrouping and on dense
+// matrices by test_stage_order...).  The step Xe Xo Ye Yo(f) Ye Xo Xe therefore equals
+// [Xe(h) Xo(f) Xe(h)] [Ye(h) Yo(f) Ye(h)], and across chained steps the adjacent half sweeps merge:
+// per pass  X: Xe(h) Xo(f) {Xe(f) Xo(f)}^(S-1) Xe(h),  Y: likewise.  4S+2 sweeps instead of 7S.
+// Only the rounding differs from the literal sequence.
+//   in : (a0, a1) = rows (yj, yj+1) entering step; (g, h) = rows (yj-2, yj-1), h waiting for Yo
+//   out: (g, h) finished with this step; (a0, a1) held for the next iteration
+template <typename T, bool PER, bool FIRST, bool LAST>
+__device__ __forceinline__ void stream_stage_nopot(const StreamParams<T>& p,
+                                                   const StreamCtx<T>& c, int yj, Row4<T>& a0,
+                                                   Row4<T>& a1, Row4<T>& g, Row4<T>& h) {
+    const T t_open = FIRST ? p.t_h : p.t_f;
+    xe(a0, t_open); xe(a1, t_open);
+    if (c.xedge) { xo<T, true>(a0, p.t_f, c.e); xo<T, true>(a1, p.t_f, c.e); }
+    else { xo<T, false>(a0, p.t_f, c.e); xo<T, false>(a1, p.t_f, c.e); }
+    if (LAST) { xe(a0, p.t_h); xe(a1, p.t_h); }
+    ypair(a0, a1, t_open);
+    const bool yedge = !PER && (yj == 0 || yj == p.ny);
+    if (yedge) { if (yj == 0) scale_row(a0, p.sec_f); else scale_row(h, p.sec_f); }
+    else ypair(h, a0, p.t_f);
+    if (LAST) ypair(g, h, p.t_h);
+}
+
+template <typename T, int S, bool POT, bool PER, int MINB>
+__global__ void __launch_bounds__(kWarps * 32, MINB)
 stream_kernel(const StreamParams<T> p) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int P = S + 1;                  // register slots = rotation period of the pipeline
@@ -153,7 +194,7 @@ stream_kernel(const StreamParams<T> p) {
     constexpr uint32_t SLOTB = NROW * ROWB;
 
     const int lane = threadIdx.x & 31;
-    const int warp = threadIdx.x >> 5;
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);   // warp-uniform
     const int strip = blockIdx.x * kWarps + warp;
     if (strip >= p.n_strips) return;
     const int NST = p.nst;
@@ -163,20 +204,22 @@ stream_kernel(const StreamParams<T> p) {
     const int xs = x0 - p.halo;               // first column of the strip window
     const int xb = xs + 4 * lane;
     StreamCtx<T> c;
-    c.xl = xb;
     c.xvalid = PER ? true : (xb >= 0 && xb < p.nx);
     c.xedge = !PER && (xs < 0 || xs + kStripSites > p.nx);
-    c.e.t_up = (xb == 0 || xb == p.nx) ? T(0) : p.t_h;
-    c.e.t_dn = (xb + 4 == p.nx || xb + 4 == 0) ? T(0) : p.t_h;
-    c.e.c0 = (xb == 0) ? p.sec_h : T(1);
-    c.e.c3 = (xb + 4 == p.nx) ? p.sec_h : T(1);
+    const T t_xo = POT ? p.t_h : p.t_f;       // X-odd sweeps are full-angle when regrouped
+    const T sec_xo = POT ? p.sec_h : p.sec_f;
+    c.e.t_up = (xb == 0 || xb == p.nx) ? T(0) : t_xo;
+    c.e.t_dn = (xb + 4 == p.nx || xb + 4 == 0) ? T(0) : t_xo;
+    c.e.c0 = (xb == 0) ? sec_xo : T(1);
+    c.e.c3 = (xb + 4 == p.nx) ? sec_xo : T(1);
     c.ring = smem_u32(smem_raw) + warp * NST * SLOTB;
     c.lane_off = lane * 4 * sizeof(T);
     const uint32_t bars = smem_u32(smem_raw) + kWarps * NST * SLOTB + warp * NST * 8;
     const bool store_ok = (4 * lane >= p.halo) && (4 * lane < kStripSites - p.halo) && (xb < p.nx);
 
-    // the strip window [xs, xs+128) as at most two contiguous global pieces (warp-uniform)
-    int gx_a, off_a, len_a, len_b;            // piece B always starts at global column 0
+    // the strip window [xs, xs+128) as at most two contiguous global pieces (warp-uniform);
+    // piece B (periodic wrap) always starts at global column 0
+    int gx_a, off_a, len_a, len_b;
     if (PER) {
         gx_a = wrap_index(xs, p.nx);
         off_a = 0;
@@ -188,48 +231,54 @@ stream_kernel(const StreamParams<T> p) {
         len_a = min(xs + kStripSites, p.nx) - gx_a;
         len_b = 0;
     }
-    const uint32_t slot_tx = NROW * (len_a + len_b) * sizeof(T);
-
-    // lane r < NROW issues the copies of row r of a slot
-    const T* my_plane = nullptr;
-    if (lane < NROW) {
-        const int plane = lane & 1, is_pot = lane >> 2;
-        my_plane = is_pot ? (plane ? p.pot_im : p.pot_re) : (plane ? p.src_im : p.src_re);
-    }
-    const int my_rowsel = (lane >> 1) & 1;
+    const uint32_t bytes_a = len_a * sizeof(T), bytes_b = len_b * sizeof(T);
+    const uint32_t slot_tx = NROW * (bytes_a + bytes_b);
+    const uint32_t dst_a = off_a * sizeof(T), dst_b = bytes_a;
 
     const int y_out0 = blockIdx.y * p.seg_rows;
     const int y_out1 = min(y_out0 + p.seg_rows, p.ny);
     const int y_in0 = y_out0 - 2 * S;
     const int n_iter = (y_out1 - y_out0) / 2 + 2 * S;
 
-    if (lane == 0) {
+    const bool leader = elect_one();
+    if (leader) {
         for (int s = 0; s < NST; ++s) mbar_init(bars + 8 * s, 1);
         mbar_fence_init();
     }
     __syncwarp();
 
-    // fetch the rows of iteration k into ring slot `slot`
-    auto issue = [&](int k, int slot) {
-        const int y = y_in0 + 2 * k;
-        const bool rowok = PER ? true : (y >= 0 && y < p.ny);
-        const int yl = PER ? wrap_index(y, p.ny) : y;
-        const uint32_t bar = bars + 8 * slot;
-        if (lane == 0) {
-            if (rowok) mbar_arrive_expect_tx(bar, slot_tx);
-            else mbar_arrive(bar);
+    // running row of the next fetch (warp-uniform): rows (fy, fy+1), element offset foff
+    int fy = PER ? wrap_index(y_in0, p.ny) : y_in0;
+    int64_t foff = (int64_t)fy * p.nx;
+    const int64_t plane_elems = (int64_t)p.nx * p.ny;
+
+    // fetch the next row pair into ring slot `slot` (one elected lane issues all copies)
+    auto issue = [&](int slot) {
+        const bool rowok = PER ? true : (fy >= 0 && fy < p.ny);
+        if (leader) {
+            const uint32_t bar = bars + 8 * slot;
+            if (rowok) {
+                mbar_arrive_expect_tx(bar, slot_tx);
+                const uint32_t dst = c.ring + slot * SLOTB;
+                const T* planes[8] = {p.src_re, p.src_im, p.src_re, p.src_im,
+                                      p.pot_re, p.pot_im, p.pot_re, p.pot_im};
+#pragma unroll
+                for (int r = 0; r < NROW; ++r) {
+                    const T* row = planes[r] + foff + ((r >> 1) & 1) * p.nx;
+                    bulk_g2s(dst + r * ROWB + dst_a, row + gx_a, bytes_a, bar);
+                    if (bytes_b) bulk_g2s(dst + r * ROWB + dst_b, row, bytes_b, bar);
+                }
+            } else {
+                mbar_arrive(bar);
+            }
         }
-        __syncwarp();
-        if (rowok && lane < NROW) {
-            const T* src = my_plane + (int64_t)(yl + my_rowsel) * p.nx;
-            const uint32_t dst = c.ring + slot * SLOTB + lane * ROWB;
-            bulk_g2s(dst + off_a * sizeof(T), src + gx_a, len_a * sizeof(T), bar);
-            if (len_b > 0) bulk_g2s(dst + len_a * sizeof(T), src, len_b * sizeof(T), bar);
-        }
+        fy += 2;
+        foff += 2 * (int64_t)p.nx;
+        if (PER && fy >= p.ny) { fy -= p.ny; foff -= plane_elems; }
     };
 
     for (int k = 0; k < DIST; ++k)
-        if (k < n_iter) issue(k, k);
+        if (k < n_iter) issue(k);
 
     Row4<T> reg[P][2];
 #pragma unroll
@@ -245,8 +294,8 @@ stream_kernel(const StreamParams<T> p) {
         for (int u = 0; u < P; ++u) {
             const int it = it0 + u;
             if (it < n_iter) {
-                __syncwarp();
-                if (it + DIST < n_iter) issue(it + DIST, rs);
+                __syncwarp();   // every lane is done with the slot about to be refilled
+                if (it + DIST < n_iter) issue(rs);
                 mbar_wait(bars + 8 * cs, cph);
                 const int y = y_in0 + 2 * it;
                 const bool rowok = PER ? true : (y >= 0 && y < p.ny);
@@ -271,10 +320,29 @@ stream_kernel(const StreamParams<T> p) {
                         pot_yj = c.ring + s0 * SLOTB + 4 * ROWB;
                         pot_yjm1 = c.ring + s1 * SLOTB + 6 * ROWB;
                     }
-                    stream_stage<T, POT, PER>(p, c, y - 2 * j, reg[(u - j + P) % P][0],
-                                              reg[(u - j + P) % P][1],
-                                              reg[(u - j - 1 + 2 * P) % P][0],
-                                              reg[(u - j - 1 + 2 * P) % P][1], pot_yj, pot_yjm1);
+                    Row4<T>& i0 = reg[(u - j + P) % P][0];
+                    Row4<T>& i1 = reg[(u - j + P) % P][1];
+                    Row4<T>& g = reg[(u - j - 1 + 2 * P) % P][0];
+                    Row4<T>& h = reg[(u - j - 1 + 2 * P) % P][1];
+                    if (POT) {
+                        if (j == 0 && j == S - 1)
+                            stream_stage<T, POT, PER, true, true>(p, c, y - 2 * j, i0, i1, g, h, pot_yj, pot_yjm1);
+                        else if (j == 0)
+                            stream_stage<T, POT, PER, true, false>(p, c, y - 2 * j, i0, i1, g, h, pot_yj, pot_yjm1);
+                        else if (j == S - 1)
+                            stream_stage<T, POT, PER, false, true>(p, c, y - 2 * j, i0, i1, g, h, pot_yj, pot_yjm1);
+                        else
+                            stream_stage<T, POT, PER, false, false>(p, c, y - 2 * j, i0, i1, g, h, pot_yj, pot_yjm1);
+                    } else {
+                        if (j == 0 && j == S - 1)
+                            stream_stage_nopot<T, PER, true, true>(p, c, y - 2 * j, i0, i1, g, h);
+                        else if (j == 0)
+                            stream_stage_nopot<T, PER, true, false>(p, c, y - 2 * j, i0, i1, g, h);
+                        else if (j == S - 1)
+                            stream_stage_nopot<T, PER, false, true>(p, c, y - 2 * j, i0, i1, g, h);
+                        else
+                            stream_stage_nopot<T, PER, false, false>(p, c, y - 2 * j, i0, i1, g, h);
+                    }
                 }
                 if (it >= 2 * S && store_ok) {
                     const Row4<T>& o0 = reg[(u - S + 2 * P) % P][0];
@@ -296,7 +364,9 @@ template <typename T, int S, bool POT, bool PER>
 int launch(const StreamParams<T>& p, cudaStream_t st) {
     constexpr uint32_t SLOTB = (POT ? 8 : 4) * kStripSites * sizeof(T);
     const size_t smem = (size_t)kWarps * p.nst * (SLOTB + 8);
-    auto kern = stream_kernel<T, S, POT, PER>;
+    // register budget: 4 blocks/SM (128 regs) for fp32, 3 (168) or 2 (255) for fp64
+    constexpr int MINB = sizeof(T) == 4 ? 4 : (S <= 2 ? 3 : 2);
+    auto kern = stream_kernel<T, S, POT, PER, MINB>;
     static size_t configured = 0;    // per instantiation
     if (smem > configured) {
         TS_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -339,7 +409,13 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
     p.sec_h = (T)(1.0 / c.a_h);
     p.sec_f = (T)(1.0 / c.a_f);
     const double per_step = pot ? pow(c.a_h, 8) : pow(c.a_h, 6) * c.a_f;
-    p.out_scale = (T)pow(per_step, S);
+    if (pot) {
+        // each of the S-1 inner step boundaries applies one Xe(f) instead of Xe(h) Xe(h)
+        p.out_scale = (T)(pow(per_step, S) * pow(c.a_f / (c.a_h * c.a_h), S - 1));
+    } else {
+        // regrouped: per axis Xe(h), S x Xo(f), (S-1) x Xe(f), Xe(h)
+        p.out_scale = (T)(pow(c.a_h, 4) * pow(c.a_f, 4 * S - 2));
+    }
     const bool per = L.periodic != 0;
     switch (S) {
         case 1: return launch_s<T, 1>(p, pot != nullptr, per, st);
@@ -359,9 +435,11 @@ bool stream_supported(const LatticeDesc& L, const StepCoef& c) {
 }
 
 int stream_default_slots(const LatticeDesc& L, int S, bool pot) {
-    // sized so that 2-4 blocks of 4 warps fit the 227 KB of an SM with >= 3 iterations in flight
-    if (L.dtype == TS_F32) return pot ? S + 4 : 6;
-    return pot ? S + 4 : 6;
+    // measured on B200 (profiles/r1b_probe.txt): 8 row-pair slots per warp keep ~7 iterations in
+    // flight for fp32 without a potential (64 KB per block, 3 blocks per SM); with a potential a
+    // slot also carries the phase rows and stays live S+1 iterations, so S+4 leaves 3 in flight.
+    if (pot) return S + 4;
+    return L.dtype == TS_F32 ? 8 : 6;
 }
 
 int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
