@@ -221,7 +221,8 @@ def run_gpu(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
     n1 = plan.norm(re, im)
-    info = {k: plan.info(k) for k in ("fused", "fuse_steps", "passes", "launches", "seg_rows")}
+    info = {k: plan.info(k) for k in ("fused", "fuse_steps", "passes", "launches", "seg_rows",
+                                     "variant")}
     value = world * cfg.sites * cfg.n_steps * args.steps / (ms * 1e-3)
 
     # end to end through ts_evolve_host: pinned host planes, H2D + D2H inside the timed region
@@ -283,7 +284,8 @@ def run_gpu(args):
         "gpu_launches": info["launches"] * args.steps,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": traffic,
-                     "kernel": f"fused_kernel<{cfg.dtype}, S={S}>",
+                     "kernel": f"{'stream_kernel' if info['variant'] == 2 else 'fused_kernel'}"
+                               f"<{cfg.dtype}, S={S}>",
                      "bytes_per_launch": bytes_per_launch, "launch_ms": launch_ms,
                      "peak_source": peak_src,
                      "site_step_roofline": peak * 1e9 / (bytes_per_launch / cfg.sites / S),

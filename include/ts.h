@@ -107,7 +107,7 @@ int ts_plan_destroy(ts_plan* plan);           /* NULL is accepted (no-op, TS_OK)
 
 const char* ts_last_error(void);              /* never NULL; "" if no failure yet */
 
-#define TS_MAX_FUSE 4
+#define TS_MAX_FUSE 6
 
 #ifdef __cplusplus
 }

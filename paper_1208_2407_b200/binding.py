@@ -8,7 +8,7 @@ from pathlib import Path
 TS_F32, TS_F64 = 0, 1
 TS_CLOSED, TS_PERIODIC = 0, 1
 TS_OK, TS_EINVAL, TS_EUNSUPPORTED, TS_EALLOC, TS_ECUDA = 0, 1, 2, 3, 4
-TS_MAX_FUSE = 4
+TS_MAX_FUSE = 6
 
 _LIB_PATH = Path(__file__).resolve().parent / "libts.so"
 _lib = None

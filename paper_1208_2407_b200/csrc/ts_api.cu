@@ -197,12 +197,18 @@ int ts_evolve(ts_plan* plan, void* psi_re, void* psi_im, double a_half, double b
     if (rc == TS_OK) rc = ensure_alloc(&plan->scratch_im, plane_bytes);
     if (rc != TS_OK) return rc;
 
-    const int S = plan->opt_fuse ? (int)plan->opt_fuse : ts::fused_default_steps(L, pot != nullptr);
-    const int seg = plan->opt_seg ? (int)plan->opt_seg : ts::fused_default_seg_rows(L, S);
     const bool can_stream = ts::stream_supported(L, c);
     if (plan->opt_variant == 2 && !can_stream)
         return fail(TS_EUNSUPPORTED, "the TMA ring kernel needs nx >= 128");
     const bool use_stream = can_stream && plan->opt_variant != 1;
+    int S = plan->opt_fuse ? (int)plan->opt_fuse : ts::fused_default_steps(L, pot != nullptr);
+    const int s_max = use_stream ? ts::stream_max_steps(L, pot != nullptr) : 4;
+    if (S > s_max) {
+        if (plan->opt_fuse)
+            return fail(TS_EUNSUPPORTED, "fuse_steps > 4 needs the TMA ring kernel, fp32, no potential");
+        S = s_max;
+    }
+    const int seg = plan->opt_seg ? (int)plan->opt_seg : ts::fused_default_seg_rows(L, S);
     plan->info_variant = use_stream ? 2 : 1;
     void* cur_re = psi_re; void* cur_im = psi_im;
     void* nxt_re = plan->scratch_re; void* nxt_im = plan->scratch_im;

@@ -255,24 +255,27 @@ bool fused_supported(const LatticeDesc& L, const StepCoef& c) {
 
 int fused_default_seg_rows(const LatticeDesc& L, int S) {
     // One warp per (strip, segment).  Aim at >= two full waves of 16 warps on 148 SMs; a segment
-    // recomputes 2S warm-up row pairs, so keep it >= 32 rows, and <= 256 (measured best on C4).
+    // recomputes 2S warm-up row pairs, so keep it >= 8 rows, and <= 256 / 512.
     const int halo = (2 * S + 3) / 4 * 4;
     const int64_t strips = (L.nx + (kStripSites - 2 * halo) - 1) / (kStripSites - 2 * halo);
     const int64_t want = 148 * 16 * 2;
     int64_t segs = (want + strips - 1) / strips;
     int64_t r = L.ny / (segs > 0 ? segs : 1);
     r -= r % 2;
-    if (r > 256) r = 256;
-    if (r < 32) r = 32;
+    // longer segments for deeper pipelines: 2S warm-up iterations per segment (probe r1d)
+    const int64_t cap = S >= 5 ? 512 : 256;
+    if (r > cap) r = cap;
+    if (r < 8) r = 8;     // small lattices: parallelism over warm-up redundancy
     if (r > L.ny) r = L.ny;
     return (int)r;
 }
 
 int fused_default_steps(const LatticeDesc& L, bool pot) {
     // steps fused per pass, measured at 16384^2 on B200 (profiles/r1b_probe.txt):
-    // fp32 no potential 4 (regrouped sweeps, HBM-bound), fp32 with potential 2, fp64 3.
-    if (L.dtype == TS_F32) return pot ? 2 : 4;
-    return 3;
+    // fp32 no potential 6 (regrouped sweeps, packed FMAs; ts_evolve clamps to what the chosen
+    // kernel has), fp32 with potential 2, fp64 3 / 4.
+    if (L.dtype == TS_F32) return pot ? 2 : 6;
+    return pot ? 3 : 4;
 }
 
 int fused_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,

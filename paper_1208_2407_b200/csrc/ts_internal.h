@@ -48,6 +48,7 @@ int fused_default_seg_rows(const LatticeDesc& L, int S);
 
 // ---- fused streaming path v2 (ts_stream.cu): TMA bulk copies into a per-warp smem ring ---------
 bool stream_supported(const LatticeDesc& L, const StepCoef& c);
+int stream_max_steps(const LatticeDesc& L, bool pot);   // 6 for fp32 without potential, else 4
 int stream_default_slots(const LatticeDesc& L, int S, bool pot);
 int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
                 void* dst_im, const StepCoef& c, const void* pot, int S, int seg_rows, int nst,

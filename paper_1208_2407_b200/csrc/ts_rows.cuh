@@ -29,8 +29,13 @@ __device__ __forceinline__ void ld4(const double* __restrict__ p, double (&v)[4]
     const double2 b = __ldg(reinterpret_cast<const double2*>(p) + 1);
     v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
 }
+__device__ __forceinline__ void mul2v(float& dx, float& dy, float ax, float ay, float bx,
+                                      float by);
 __device__ __forceinline__ void st4(float* __restrict__ p, const float (&v)[4], float s) {
-    *reinterpret_cast<float4*>(p) = make_float4(v[0] * s, v[1] * s, v[2] * s, v[3] * s);
+    float4 q;
+    mul2v(q.x, q.y, v[0], v[1], s, s);
+    mul2v(q.z, q.w, v[2], v[3], s, s);
+    *reinterpret_cast<float4*>(p) = q;
 }
 __device__ __forceinline__ void st4(double* __restrict__ p, const double (&v)[4], double s) {
     reinterpret_cast<double2*>(p)[0] = make_double2(v[0] * s, v[1] * s);
@@ -53,12 +58,58 @@ __device__ __forceinline__ void rot(T& rp, T& ip, T& rq, T& iq, T t) {
     rp = nrp; ip = nip; rq = nrq; iq = niq;
 }
 
+// Packed fp32 arithmetic (sm_100: fma.rn.f32x2 / mul.rn.f32x2, SASS FFMA2 / FMUL2): two FMAs per
+// issue slot on an aligned register pair.  The kernel is issue-limited before it is FMA-pipe
+// limited (profiles/r1b_*), so the sweeps whose pairs line up with adjacent sites use it.  ptxas
+// folds the scalar broadcast, the negation and a swapped source pair into operand modifiers.
+// (dx, dy) = s * (bx, by) + (cx, cy)
+__device__ __forceinline__ void fma2(float& dx, float& dy, float s, float bx, float by, float cx,
+                                     float cy) {
+    unsigned long long rs, rb, rc, rd;
+    asm("mov.b64 %0, {%1, %1};" : "=l"(rs) : "f"(s));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(rb) : "f"(bx), "f"(by));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(rc) : "f"(cx), "f"(cy));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(rd) : "l"(rs), "l"(rb), "l"(rc));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(dx), "=f"(dy) : "l"(rd));
+}
+// (dx, dy) = (ax, ay) * (bx, by) + (cx, cy)
+__device__ __forceinline__ void fma2v(float& dx, float& dy, float ax, float ay, float bx, float by,
+                                      float cx, float cy) {
+    unsigned long long ra, rb, rc, rd;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ra) : "f"(ax), "f"(ay));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(rb) : "f"(bx), "f"(by));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(rc) : "f"(cx), "f"(cy));
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(rd) : "l"(ra), "l"(rb), "l"(rc));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(dx), "=f"(dy) : "l"(rd));
+}
+// (dx, dy) = (ax, ay) * (bx, by)
+__device__ __forceinline__ void mul2v(float& dx, float& dy, float ax, float ay, float bx,
+                                      float by) {
+    unsigned long long ra, rb, rd;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(ra) : "f"(ax), "f"(ay));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(rb) : "f"(bx), "f"(by));
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(rd) : "l"(ra), "l"(rb));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(dx), "=f"(dy) : "l"(rd));
+}
+
 // X-even sweep on one row: pairs (0,1), (2,3) of the lane's four sites
 template <typename T>
 __device__ __forceinline__ void xe(Row4<T>& r, T t) {
     rot(r.re[0], r.im[0], r.re[1], r.im[1], t);
     rot(r.re[2], r.im[2], r.re[3], r.im[3], t);
 }
+#ifndef TS_SCALAR_F32   // -DTS_SCALAR_F32: A/B build without the packed forms
+// fp32: (re_k, re_k+1) -= t (im_k+1, im_k); (im_k, im_k+1) += t (re_k+1, re_k)   [old values]
+__device__ __forceinline__ void xe(Row4<float>& r, float t) {
+#pragma unroll
+    for (int k = 0; k < 4; k += 2) {
+        float nr0, nr1, ni0, ni1;
+        fma2(nr0, nr1, -t, r.im[k + 1], r.im[k], r.re[k], r.re[k + 1]);
+        fma2(ni0, ni1, t, r.re[k + 1], r.re[k], r.im[k], r.im[k + 1]);
+        r.re[k] = nr0; r.re[k + 1] = nr1; r.im[k] = ni0; r.im[k + 1] = ni1;
+    }
+}
+#endif
 
 // per-lane coefficients of the cross-lane X-odd pair; differ from (t, t, 1, 1) only in strips
 // that touch a closed domain edge
@@ -101,6 +152,21 @@ __device__ __forceinline__ void ypair(Row4<T>& a, Row4<T>& b, T t) {
     for (int i = 0; i < 4; ++i) rot(a.re[i], a.im[i], b.re[i], b.im[i], t);
 }
 
+#ifndef TS_SCALAR_F32
+__device__ __forceinline__ void ypair(Row4<float>& a, Row4<float>& b, float t) {
+#pragma unroll
+    for (int k = 0; k < 4; k += 2) {
+        float ar0, ar1, ai0, ai1, br0, br1, bi0, bi1;
+        fma2(ar0, ar1, -t, b.im[k], b.im[k + 1], a.re[k], a.re[k + 1]);
+        fma2(ai0, ai1, t, b.re[k], b.re[k + 1], a.im[k], a.im[k + 1]);
+        fma2(br0, br1, -t, a.im[k], a.im[k + 1], b.re[k], b.re[k + 1]);
+        fma2(bi0, bi1, t, a.re[k], a.re[k + 1], b.im[k], b.im[k + 1]);
+        a.re[k] = ar0; a.re[k + 1] = ar1; a.im[k] = ai0; a.im[k + 1] = ai1;
+        b.re[k] = br0; b.re[k + 1] = br1; b.im[k] = bi0; b.im[k + 1] = bi1;
+    }
+}
+#endif
+
 template <typename T>
 __device__ __forceinline__ void scale_row(Row4<T>& r, T s) {
 #pragma unroll
@@ -117,6 +183,21 @@ __device__ __forceinline__ void phase_row(Row4<T>& r, const T (&pr)[4], const T 
         r.im[i] = fma(b, pr[i], a * pi[i]);
     }
 }
+
+#ifndef TS_SCALAR_F32
+__device__ __forceinline__ void phase_row(Row4<float>& r, const float (&pr)[4],
+                                          const float (&pi)[4]) {
+#pragma unroll
+    for (int k = 0; k < 4; k += 2) {
+        float m0, m1, n0, n1, nr0, nr1, ni0, ni1;
+        mul2v(m0, m1, r.re[k], r.re[k + 1], pr[k], pr[k + 1]);
+        mul2v(n0, n1, r.re[k], r.re[k + 1], pi[k], pi[k + 1]);
+        fma2v(nr0, nr1, -r.im[k], -r.im[k + 1], pi[k], pi[k + 1], m0, m1);
+        fma2v(ni0, ni1, r.im[k], r.im[k + 1], pr[k], pr[k + 1], n0, n1);
+        r.re[k] = nr0; r.re[k + 1] = nr1; r.im[k] = ni0; r.im[k + 1] = ni1;
+    }
+}
+#endif
 
 __device__ __forceinline__ int wrap_index(int v, int n) {
     while (v < 0) v += n;

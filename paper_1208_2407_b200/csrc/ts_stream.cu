@@ -25,6 +25,10 @@ using namespace rows;
 
 constexpr int kWarps = 4;
 
+#ifndef TS_STREAM_ROLLED
+#define TS_STREAM_ROLLED 1
+#endif
+
 template <typename T>
 struct StreamParams {
     const T* src_re;
@@ -238,7 +242,13 @@ stream_kernel(const StreamParams<T> p) {
     const int y_out0 = blockIdx.y * p.seg_rows;
     const int y_out1 = min(y_out0 + p.seg_rows, p.ny);
     const int y_in0 = y_out0 - 2 * S;
+#if TS_STREAM_ROLLED
+    // even, so that the two-iteration loop body has no conditional half (the extra iteration only
+    // feeds the pipeline; its output row pair lies beyond the segment and is not stored)
+    const int n_iter = ((y_out1 - y_out0) / 2 + 2 * S + 1) & ~1;
+#else
     const int n_iter = (y_out1 - y_out0) / 2 + 2 * S;
+#endif
 
     const bool leader = elect_one();
     if (leader) {
@@ -280,13 +290,98 @@ stream_kernel(const StreamParams<T> p) {
     for (int k = 0; k < DIST; ++k)
         if (k < n_iter) issue(k);
 
-    Row4<T> reg[P][2];
-#pragma unroll
-    for (int s = 0; s < P; ++s) { zero_row(reg[s][0]); zero_row(reg[s][1]); }
-
     int cs = 0;                 // ring slot of the current iteration
     uint32_t cph = 0;           // its mbarrier phase parity
     int rs = DIST % NST;        // ring slot refilled at the top of the current iteration
+
+#if TS_STREAM_ROLLED
+    // Ping-pong form of the pipeline.  Stage j owns two register sets W[j][0], W[j][1]: in an
+    // even iteration the incoming pair is written to set 0 and the pair that waited there since
+    // the previous iteration for its vertical-odd partner is set 1, in an odd iteration the other
+    // way round.  The pair that leaves stage j is handed to stage j+1 by value (the copy folds
+    // into the first sweep of that stage), and a set is dead once its pair has left, so S+1 pairs
+    // are live, exactly as in a rotation over S+1 sets -- but the loop repeats after TWO iterations
+    // instead of S+1: the S+1-fold unrolled rotation of r1b was 41 KB of SASS at S = 4 and
+    // overflowed the instruction cache beyond (no_instruction stalls, profiles/r1d_*).
+    Row4<T> W[S][2][2];
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+        zero_row(W[s][0][0]); zero_row(W[s][0][1]); zero_row(W[s][1][0]); zero_row(W[s][1][1]);
+    }
+
+#pragma unroll 1
+    for (int it0 = 0; it0 < n_iter; it0 += 2) {
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const int it = it0 + u;
+            {
+                __syncwarp();   // every lane is done with the slot about to be refilled
+                if (it + DIST < n_iter) issue(rs);
+                mbar_wait(bars + 8 * cs, cph);
+                const int y = y_in0 + 2 * it;
+                const bool rowok = PER ? true : (y >= 0 && y < p.ny);
+                Row4<T> x0, x1;
+                if (rowok && c.xvalid) {
+                    const uint32_t base = c.ring + cs * SLOTB + c.lane_off;
+                    lds4(base, x0.re);
+                    lds4(base + ROWB, x0.im);
+                    lds4(base + 2 * ROWB, x1.re);
+                    lds4(base + 3 * ROWB, x1.im);
+                } else {
+                    zero_row(x0);
+                    zero_row(x1);
+                }
+#pragma unroll
+                for (int j = 0; j < S; ++j) {
+                    uint32_t pot_yj = 0, pot_yjm1 = 0;
+                    if (POT) {
+                        int s0 = cs - j;      if (s0 < 0) s0 += NST;
+                        int s1 = s0 - 1;      if (s1 < 0) s1 += NST;
+                        pot_yj = c.ring + s0 * SLOTB + 4 * ROWB;
+                        pot_yjm1 = c.ring + s1 * SLOTB + 6 * ROWB;
+                    }
+                    Row4<T>& a0 = W[j][u][0];
+                    Row4<T>& a1 = W[j][u][1];
+                    Row4<T>& g = W[j][u ^ 1][0];
+                    Row4<T>& h = W[j][u ^ 1][1];
+                    a0 = x0; a1 = x1;
+                    if (POT) {
+                        if (j == 0 && j == S - 1)
+                            stream_stage<T, POT, PER, true, true>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
+                        else if (j == 0)
+                            stream_stage<T, POT, PER, true, false>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
+                        else if (j == S - 1)
+                            stream_stage<T, POT, PER, false, true>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
+                        else
+                            stream_stage<T, POT, PER, false, false>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
+                    } else {
+                        if (j == 0 && j == S - 1)
+                            stream_stage_nopot<T, PER, true, true>(p, c, y - 2 * j, a0, a1, g, h);
+                        else if (j == 0)
+                            stream_stage_nopot<T, PER, true, false>(p, c, y - 2 * j, a0, a1, g, h);
+                        else if (j == S - 1)
+                            stream_stage_nopot<T, PER, false, true>(p, c, y - 2 * j, a0, a1, g, h);
+                        else
+                            stream_stage_nopot<T, PER, false, false>(p, c, y - 2 * j, a0, a1, g, h);
+                    }
+                    x0 = g; x1 = h;
+                }
+                if (it >= 2 * S && store_ok && y - 2 * S < y_out1) {
+                    const int64_t off = (int64_t)(y - 2 * S) * p.nx + xb;
+                    st4(p.dst_re + off, x0.re, p.out_scale);
+                    st4(p.dst_im + off, x0.im, p.out_scale);
+                    st4(p.dst_re + off + p.nx, x1.re, p.out_scale);
+                    st4(p.dst_im + off + p.nx, x1.im, p.out_scale);
+                }
+                if (++cs == NST) { cs = 0; cph ^= 1; }
+                if (++rs == NST) rs = 0;
+            }
+        }
+    }
+#else
+    Row4<T> reg[P][2];
+#pragma unroll
+    for (int s = 0; s < P; ++s) { zero_row(reg[s][0]); zero_row(reg[s][1]); }
 
 #pragma unroll 1
     for (int it0 = 0; it0 < n_iter; it0 += P) {
@@ -358,14 +453,19 @@ stream_kernel(const StreamParams<T> p) {
             }
         }
     }
+#endif
 }
 
 template <typename T, int S, bool POT, bool PER>
 int launch(const StreamParams<T>& p, cudaStream_t st) {
     constexpr uint32_t SLOTB = (POT ? 8 : 4) * kStripSites * sizeof(T);
     const size_t smem = (size_t)kWarps * p.nst * (SLOTB + 8);
-    // register budget: 4 blocks/SM (128 regs) for fp32, 3 (168) or 2 (255) for fp64
-    constexpr int MINB = sizeof(T) == 4 ? 4 : (S <= 2 ? 3 : 2);
+    // register budget: 4 blocks/SM (128 regs) for fp32 up to S = 4, 3 (168) beyond; 3 or 2 (255)
+    // for fp64
+#ifndef TS_MINB_F32
+#define TS_MINB_F32 (S <= 4 ? 4 : 3)
+#endif
+    constexpr int MINB = sizeof(T) == 4 ? TS_MINB_F32 : (S <= 2 ? 3 : 2);
     auto kern = stream_kernel<T, S, POT, PER, MINB>;
     static size_t configured = 0;    // per instantiation
     if (smem > configured) {
@@ -423,6 +523,13 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
         case 3: return launch_s<T, 3>(p, pot != nullptr, per, st);
         case 4: return launch_s<T, 4>(p, pot != nullptr, per, st);
     }
+    // deeper temporal blocking only where the ALU budget allows it: fp32 without a potential
+    if constexpr (sizeof(T) == 4) {
+        if (!pot) {
+            if (S == 5) return per ? launch<T, 5, false, true>(p, st) : launch<T, 5, false, false>(p, st);
+            if (S == 6) return per ? launch<T, 6, false, true>(p, st) : launch<T, 6, false, false>(p, st);
+        }
+    }
     set_error("stream_pass: steps per pass out of range");
     return TS_EINVAL;
 }
@@ -432,6 +539,10 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
 bool stream_supported(const LatticeDesc& L, const StepCoef& c) {
     // the strip window must split into at most two contiguous pieces of a row
     return fused_supported(L, c) && L.nx >= kStripSites;
+}
+
+int stream_max_steps(const LatticeDesc& L, bool pot) {
+    return (L.dtype == TS_F32 && !pot) ? 6 : 4;
 }
 
 int stream_default_slots(const LatticeDesc& L, int S, bool pot) {
