@@ -254,15 +254,16 @@ bool fused_supported(const LatticeDesc& L, const StepCoef& c) {
 }
 
 int fused_default_seg_rows(const LatticeDesc& L, int S) {
-    // One warp per (strip, segment).  Aim at >= two full waves of 16 warps on 148 SMs; a segment
-    // recomputes 2S warm-up row pairs, so keep it >= 8 rows, and <= 256 / 512.
+    // One warp per (strip, segment); a segment recomputes 2S warm-up row pairs, so its cost is
+    // seg/2 + 2S iterations.  With W = strips * segments warps and room for ~12 warps on each of
+    // 148 SMs, time ~ max(W, 1776) * (seg/2 + 2S): longer segments win until the grid no longer
+    // fills the machine, so aim at one wave (probes r1d: 4096^2 best at ~92 rows, 16384^2 at
+    // 256 for S <= 4 and 512 beyond, 1024^2 at the lower clamp).
     const int halo = (2 * S + 3) / 4 * 4;
     const int64_t strips = (L.nx + (kStripSites - 2 * halo) - 1) / (kStripSites - 2 * halo);
-    const int64_t want = 148 * 16 * 2;
-    int64_t segs = (want + strips - 1) / strips;
-    int64_t r = L.ny / (segs > 0 ? segs : 1);
+    const int64_t want = 148 * 12;
+    int64_t r = L.ny * strips / want;
     r -= r % 2;
-    // longer segments for deeper pipelines: 2S warm-up iterations per segment (probe r1d)
     const int64_t cap = S >= 5 ? 512 : 256;
     if (r > cap) r = cap;
     if (r < 8) r = 8;     // small lattices: parallelism over warm-up redundancy
@@ -271,10 +272,14 @@ int fused_default_seg_rows(const LatticeDesc& L, int S) {
 }
 
 int fused_default_steps(const LatticeDesc& L, bool pot) {
-    // steps fused per pass, measured at 16384^2 on B200 (profiles/r1b_probe.txt):
-    // fp32 no potential 6 (regrouped sweeps, packed FMAs; ts_evolve clamps to what the chosen
-    // kernel has), fp32 with potential 2, fp64 3 / 4.
-    if (L.dtype == TS_F32) return pot ? 2 : 6;
+    // steps fused per pass, measured on B200 (profiles/r1d_probe.txt): fp32 without potential 6
+    // (regrouped sweeps, packed FMAs; ts_evolve clamps to what the chosen kernel has) -- 4 on
+    // small lattices, where segments are short and the 2S warm-up iterations dominate; fp32 with
+    // potential 3; fp64 3 with, 4 without.
+    if (L.dtype == TS_F32) {
+        if (pot) return 3;
+        return L.nx * L.ny < (int64_t(1) << 22) ? 4 : 6;
+    }
     return pot ? 3 : 4;
 }
 

@@ -15,6 +15,8 @@
 // (PAPER.md:115).
 #include <math.h>
 
+#include <type_traits>
+
 #include "ts_internal.h"
 #include "ts_rows.cuh"
 
@@ -25,9 +27,6 @@ using namespace rows;
 
 constexpr int kWarps = 4;
 
-#ifndef TS_STREAM_ROLLED
-#define TS_STREAM_ROLLED 1
-#endif
 
 template <typename T>
 struct StreamParams {
@@ -120,28 +119,23 @@ struct StreamCtx {
 // start of the later step (the deferred cos factor is adjusted in out_scale).
 // pot_yj / pot_yjm1: shared addresses of the potential rows yj (row 0 of its slot) and yj-1
 // (row 1 of the previous slot), valid when POT.
-template <typename T, bool POT, bool PER, bool FIRST, bool LAST>
+template <typename T, bool POT, bool PER, bool XEDGE, bool FIRST, bool LAST>
 __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const StreamCtx<T>& c,
                                              int yj, Row4<T>& a0, Row4<T>& a1, Row4<T>& g,
                                              Row4<T>& h, uint32_t pot_yj, uint32_t pot_yjm1) {
     constexpr uint32_t ROWB = kStripSites * sizeof(T);
     const T t_open = FIRST ? p.t_h : p.t_f;
     xe(a0, t_open); xe(a1, t_open);
-    if (c.xedge) { xo<T, true>(a0, p.t_h, c.e); xo<T, true>(a1, p.t_h, c.e); }
-    else { xo<T, false>(a0, p.t_h, c.e); xo<T, false>(a1, p.t_h, c.e); }
+    xo<T, XEDGE>(a0, p.t_h, c.e); xo<T, XEDGE>(a1, p.t_h, c.e);
     ypair(a0, a1, p.t_h);
-    const bool yedge = !PER && (yj == 0 || yj == p.ny);
-    if (!POT) {
-        if (yedge) { if (yj == 0) scale_row(a0, p.sec_f); else scale_row(h, p.sec_f); }
-        else ypair(h, a0, p.t_f);
-    } else {
-        if (yedge) {
-            if (yj == 0) scale_row(a0, p.sec_h * p.sec_h); else scale_row(h, p.sec_h * p.sec_h);
-        } else {
-            ypair(h, a0, p.t_h);
-        }
-        const bool lo_ok = c.xvalid && (PER || (yj - 1 >= 0 && yj - 1 < p.ny));
-        const bool hi_ok = c.xvalid && (PER || (yj >= 0 && yj < p.ny));
+    // closed lattice: the vertical-odd pair (yj-1, yj) does not exist at yj = 0 and yj = ny; the
+    // ghost row is zero and stays zero (coupling 0), the real row takes 1/a per omitted sweep
+    const bool yedge = XEDGE && (yj == 0 || yj == p.ny);
+    const T t_yo = yedge ? T(0) : p.t_h;
+    ypair(h, a0, t_yo);
+    {
+        const bool lo_ok = !XEDGE || (c.xvalid && yj - 1 >= 0 && yj - 1 < p.ny);
+        const bool hi_ok = !XEDGE || (c.xvalid && yj >= 0 && yj < p.ny);
         if (lo_ok) {
             T pr[4], pi[4];
             lds4(pot_yjm1 + c.lane_off, pr);
@@ -154,11 +148,14 @@ __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const Str
             lds4(pot_yj + ROWB + c.lane_off, pi);
             phase_row(a0, pr, pi);
         }
-        if (!yedge) ypair(h, a0, p.t_h);
+    }
+    ypair(h, a0, t_yo);
+    if (XEDGE) {
+        const T sy = yedge ? p.sec_h * p.sec_h : T(1);
+        scale_row(h, sy); scale_row(a0, sy);
     }
     ypair(g, h, p.t_h);
-    if (c.xedge) { xo<T, true>(g, p.t_h, c.e); xo<T, true>(h, p.t_h, c.e); }
-    else { xo<T, false>(g, p.t_h, c.e); xo<T, false>(h, p.t_h, c.e); }
+    xo<T, XEDGE>(g, p.t_h, c.e); xo<T, XEDGE>(h, p.t_h, c.e);
     if (LAST) { xe(g, p.t_h); xe(h, p.t_h); }
 }
 
@@ -171,19 +168,21 @@ __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const Str
 // Only the rounding differs from the literal sequence.
 //   in : (a0, a1) = rows (yj, yj+1) entering step; (g, h) = rows (yj-2, yj-1), h waiting for Yo
 //   out: (g, h) finished with this step; (a0, a1) held for the next iteration
-template <typename T, bool PER, bool FIRST, bool LAST>
+template <typename T, bool PER, bool XEDGE, bool FIRST, bool LAST>
 __device__ __forceinline__ void stream_stage_nopot(const StreamParams<T>& p,
                                                    const StreamCtx<T>& c, int yj, Row4<T>& a0,
                                                    Row4<T>& a1, Row4<T>& g, Row4<T>& h) {
     const T t_open = FIRST ? p.t_h : p.t_f;
     xe(a0, t_open); xe(a1, t_open);
-    if (c.xedge) { xo<T, true>(a0, p.t_f, c.e); xo<T, true>(a1, p.t_f, c.e); }
-    else { xo<T, false>(a0, p.t_f, c.e); xo<T, false>(a1, p.t_f, c.e); }
+    xo<T, XEDGE>(a0, p.t_f, c.e); xo<T, XEDGE>(a1, p.t_f, c.e);
     if (LAST) { xe(a0, p.t_h); xe(a1, p.t_h); }
     ypair(a0, a1, t_open);
-    const bool yedge = !PER && (yj == 0 || yj == p.ny);
-    if (yedge) { if (yj == 0) scale_row(a0, p.sec_f); else scale_row(h, p.sec_f); }
-    else ypair(h, a0, p.t_f);
+    // closed lattice: the vertical-odd pair (yj-1, yj) does not exist at yj = 0 and yj = ny; the
+    // real row of the two takes 1/a instead (the ghost row is zero and stays zero)
+    const bool yedge = XEDGE && (yj == 0 || yj == p.ny);
+    const T t_yo = yedge ? T(0) : p.t_f;
+    ypair(h, a0, t_yo);
+    if (XEDGE) { const T sy = yedge ? p.sec_f : T(1); scale_row(h, sy); scale_row(a0, sy); }
     if (LAST) ypair(g, h, p.t_h);
 }
 
@@ -191,7 +190,6 @@ template <typename T, int S, bool POT, bool PER, int MINB>
 __global__ void __launch_bounds__(kWarps * 32, MINB)
 stream_kernel(const StreamParams<T> p) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    constexpr int P = S + 1;                  // register slots = rotation period of the pipeline
     constexpr int R = POT ? S + 1 : 1;        // iterations a ring slot stays live after its arrival
     constexpr uint32_t ROWB = kStripSites * sizeof(T);
     constexpr int NROW = POT ? 8 : 4;         // re0 im0 re1 im1 [pr0 pi0 pr1 pi1]
@@ -242,13 +240,9 @@ stream_kernel(const StreamParams<T> p) {
     const int y_out0 = blockIdx.y * p.seg_rows;
     const int y_out1 = min(y_out0 + p.seg_rows, p.ny);
     const int y_in0 = y_out0 - 2 * S;
-#if TS_STREAM_ROLLED
     // even, so that the two-iteration loop body has no conditional half (the extra iteration only
     // feeds the pipeline; its output row pair lies beyond the segment and is not stored)
     const int n_iter = ((y_out1 - y_out0) / 2 + 2 * S + 1) & ~1;
-#else
-    const int n_iter = (y_out1 - y_out0) / 2 + 2 * S;
-#endif
 
     const bool leader = elect_one();
     if (leader) {
@@ -294,7 +288,6 @@ stream_kernel(const StreamParams<T> p) {
     uint32_t cph = 0;           // its mbarrier phase parity
     int rs = DIST % NST;        // ring slot refilled at the top of the current iteration
 
-#if TS_STREAM_ROLLED
     // Ping-pong form of the pipeline.  Stage j owns two register sets W[j][0], W[j][1]: in an
     // even iteration the incoming pair is written to set 0 and the pair that waited there since
     // the previous iteration for its vertical-odd partner is set 1, in an odd iteration the other
@@ -303,6 +296,12 @@ stream_kernel(const StreamParams<T> p) {
     // are live, exactly as in a rotation over S+1 sets -- but the loop repeats after TWO iterations
     // instead of S+1: the S+1-fold unrolled rotation of r1b was 41 KB of SASS at S = 4 and
     // overflowed the instruction cache beyond (no_instruction stalls, profiles/r1d_*).
+    // The whole loop exists twice for closed lattices: warps whose strip touches an edge in x or
+    // whose segment touches one in y (the outer ring of the warp grid) carry per-lane couplings,
+    // zero ghost sites and the 1/a factor of unpaired sites (XEDGE, branch-free selects); all
+    // others run the unmodified sweeps.  Chosen once per warp: no branch inside the sweeps.
+    auto run = [&](auto xedge_tag) {
+    constexpr bool XEDGE = decltype(xedge_tag)::value;
     Row4<T> W[S][2][2];
 #pragma unroll
     for (int s = 0; s < S; ++s) {
@@ -319,9 +318,9 @@ stream_kernel(const StreamParams<T> p) {
                 if (it + DIST < n_iter) issue(rs);
                 mbar_wait(bars + 8 * cs, cph);
                 const int y = y_in0 + 2 * it;
-                const bool rowok = PER ? true : (y >= 0 && y < p.ny);
+                const bool rowok = !XEDGE || (y >= 0 && y < p.ny && c.xvalid);
                 Row4<T> x0, x1;
-                if (rowok && c.xvalid) {
+                if (rowok) {
                     const uint32_t base = c.ring + cs * SLOTB + c.lane_off;
                     lds4(base, x0.re);
                     lds4(base + ROWB, x0.im);
@@ -347,22 +346,22 @@ stream_kernel(const StreamParams<T> p) {
                     a0 = x0; a1 = x1;
                     if (POT) {
                         if (j == 0 && j == S - 1)
-                            stream_stage<T, POT, PER, true, true>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
+                            stream_stage<T, POT, PER, XEDGE, true, true>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
                         else if (j == 0)
-                            stream_stage<T, POT, PER, true, false>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
+                            stream_stage<T, POT, PER, XEDGE, true, false>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
                         else if (j == S - 1)
-                            stream_stage<T, POT, PER, false, true>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
+                            stream_stage<T, POT, PER, XEDGE, false, true>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
                         else
-                            stream_stage<T, POT, PER, false, false>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
+                            stream_stage<T, POT, PER, XEDGE, false, false>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
                     } else {
                         if (j == 0 && j == S - 1)
-                            stream_stage_nopot<T, PER, true, true>(p, c, y - 2 * j, a0, a1, g, h);
+                            stream_stage_nopot<T, PER, XEDGE, true, true>(p, c, y - 2 * j, a0, a1, g, h);
                         else if (j == 0)
-                            stream_stage_nopot<T, PER, true, false>(p, c, y - 2 * j, a0, a1, g, h);
+                            stream_stage_nopot<T, PER, XEDGE, true, false>(p, c, y - 2 * j, a0, a1, g, h);
                         else if (j == S - 1)
-                            stream_stage_nopot<T, PER, false, true>(p, c, y - 2 * j, a0, a1, g, h);
+                            stream_stage_nopot<T, PER, XEDGE, false, true>(p, c, y - 2 * j, a0, a1, g, h);
                         else
-                            stream_stage_nopot<T, PER, false, false>(p, c, y - 2 * j, a0, a1, g, h);
+                            stream_stage_nopot<T, PER, XEDGE, false, false>(p, c, y - 2 * j, a0, a1, g, h);
                     }
                     x0 = g; x1 = h;
                 }
@@ -378,82 +377,10 @@ stream_kernel(const StreamParams<T> p) {
             }
         }
     }
-#else
-    Row4<T> reg[P][2];
-#pragma unroll
-    for (int s = 0; s < P; ++s) { zero_row(reg[s][0]); zero_row(reg[s][1]); }
-
-#pragma unroll 1
-    for (int it0 = 0; it0 < n_iter; it0 += P) {
-#pragma unroll
-        for (int u = 0; u < P; ++u) {
-            const int it = it0 + u;
-            if (it < n_iter) {
-                __syncwarp();   // every lane is done with the slot about to be refilled
-                if (it + DIST < n_iter) issue(rs);
-                mbar_wait(bars + 8 * cs, cph);
-                const int y = y_in0 + 2 * it;
-                const bool rowok = PER ? true : (y >= 0 && y < p.ny);
-                Row4<T>& a0 = reg[u][0];
-                Row4<T>& a1 = reg[u][1];
-                if (rowok && c.xvalid) {
-                    const uint32_t base = c.ring + cs * SLOTB + c.lane_off;
-                    lds4(base, a0.re);
-                    lds4(base + ROWB, a0.im);
-                    lds4(base + 2 * ROWB, a1.re);
-                    lds4(base + 3 * ROWB, a1.im);
-                } else {
-                    zero_row(a0);
-                    zero_row(a1);
-                }
-#pragma unroll
-                for (int j = 0; j < S; ++j) {
-                    uint32_t pot_yj = 0, pot_yjm1 = 0;
-                    if (POT) {
-                        int s0 = cs - j;      if (s0 < 0) s0 += NST;
-                        int s1 = s0 - 1;      if (s1 < 0) s1 += NST;
-                        pot_yj = c.ring + s0 * SLOTB + 4 * ROWB;
-                        pot_yjm1 = c.ring + s1 * SLOTB + 6 * ROWB;
-                    }
-                    Row4<T>& i0 = reg[(u - j + P) % P][0];
-                    Row4<T>& i1 = reg[(u - j + P) % P][1];
-                    Row4<T>& g = reg[(u - j - 1 + 2 * P) % P][0];
-                    Row4<T>& h = reg[(u - j - 1 + 2 * P) % P][1];
-                    if (POT) {
-                        if (j == 0 && j == S - 1)
-                            stream_stage<T, POT, PER, true, true>(p, c, y - 2 * j, i0, i1, g, h, pot_yj, pot_yjm1);
-                        else if (j == 0)
-                            stream_stage<T, POT, PER, true, false>(p, c, y - 2 * j, i0, i1, g, h, pot_yj, pot_yjm1);
-                        else if (j == S - 1)
-                            stream_stage<T, POT, PER, false, true>(p, c, y - 2 * j, i0, i1, g, h, pot_yj, pot_yjm1);
-                        else
-                            stream_stage<T, POT, PER, false, false>(p, c, y - 2 * j, i0, i1, g, h, pot_yj, pot_yjm1);
-                    } else {
-                        if (j == 0 && j == S - 1)
-                            stream_stage_nopot<T, PER, true, true>(p, c, y - 2 * j, i0, i1, g, h);
-                        else if (j == 0)
-                            stream_stage_nopot<T, PER, true, false>(p, c, y - 2 * j, i0, i1, g, h);
-                        else if (j == S - 1)
-                            stream_stage_nopot<T, PER, false, true>(p, c, y - 2 * j, i0, i1, g, h);
-                        else
-                            stream_stage_nopot<T, PER, false, false>(p, c, y - 2 * j, i0, i1, g, h);
-                    }
-                }
-                if (it >= 2 * S && store_ok) {
-                    const Row4<T>& o0 = reg[(u - S + 2 * P) % P][0];
-                    const Row4<T>& o1 = reg[(u - S + 2 * P) % P][1];
-                    const int64_t off = (int64_t)(y - 2 * S) * p.nx + xb;
-                    st4(p.dst_re + off, o0.re, p.out_scale);
-                    st4(p.dst_im + off, o0.im, p.out_scale);
-                    st4(p.dst_re + off + p.nx, o1.re, p.out_scale);
-                    st4(p.dst_im + off + p.nx, o1.im, p.out_scale);
-                }
-                if (++cs == NST) { cs = 0; cph ^= 1; }
-                if (++rs == NST) rs = 0;
-            }
-        }
-    }
-#endif
+    };   // run
+    const bool edge = !PER && (c.xedge || y_in0 < 0 || y_in0 + 2 * n_iter >= p.ny);
+    if (edge) run(std::true_type{});
+    else run(std::false_type{});
 }
 
 template <typename T, int S, bool POT, bool PER>

@@ -51,6 +51,22 @@ def test_fused_f32(nx, ny, boundary, with_pot, fuse, variant):
     assert info["passes"] == math.ceil(9 / fuse)
 
 
+@pytest.mark.parametrize("boundary", ["closed", "periodic"])
+@pytest.mark.parametrize("with_pot", [False, True])
+@pytest.mark.parametrize("dtype,fuse,seg", [("f32", 6, 8), ("f32", 4, 4), ("f32", 3, 2), ("f64", 4, 6),
+                                            ("f64", 2, 2)])
+def test_short_segments_whose_warmup_reaches_past_the_edge(boundary, with_pot, dtype, fuse, seg):
+    # segments shorter than the 2S warm-up rows: several segments start above row 0 / end below
+    # row ny-1, and in a closed lattice all of them must take the edge variant of the loop
+    if with_pot and fuse > 4:
+        pytest.skip("S = 5, 6 exist only without a potential")
+    nx, ny = 260, 44
+    cfg = G.make_cfg(nx, ny, dtype, boundary, 0.3, 13)
+    re, im, pot = G.random_inputs(nx, ny, dtype, 4242 + fuse, with_pot)
+    info = check(cfg, re, im, pot, 13, path=2, fuse=fuse, seg_rows=seg, variant=2)
+    assert info["fused"] == 1 and info["seg_rows"] == seg
+
+
 @pytest.mark.parametrize("nx,ny", [(8, 6), (124, 34), (128, 40), (252, 66), (380, 130)])
 @pytest.mark.parametrize("boundary", ["closed", "periodic"])
 @pytest.mark.parametrize("with_pot", [False, True])
