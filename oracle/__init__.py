@@ -114,6 +114,37 @@ def evolve(re, im, a_half, b_half, a_full, b_full, pot=None, periodic=False, n_s
                           _ptr(pr), _ptr(pi), int(bool(periodic)), int(n_steps))
 
 
+# p of Eq. 4: p = (4 - 4^(1/3))^-1
+U4_P = 1.0 / (4.0 - 4.0 ** (1.0 / 3.0))
+
+
+def u4_fractions():
+    """Time fractions of the five second-order sub-steps of Eq. 4, in order of application."""
+    return (U4_P, U4_P, 1.0 - 4.0 * U4_P, U4_P, U4_P)
+
+
+def evolve_u4(re, im, theta, pot_p=None, pot_q=None, periodic=False, n_steps=1) -> None:
+    """In place: n_steps fourth-order steps, Eq. 4 of the paper written out:
+
+        U4(dt) = U2(p dt) U2(p dt) U2((1-4p) dt) U2(p dt) U2(p dt),   p = (4 - 4^(1/3))^-1.
+
+    Each U2(f dt) is ``evolve`` (the pinned second-order step) with angle f*theta, i.e.
+    coefficients cos/sin(f theta/2) and cos/sin(f theta); the sequence is a palindrome, so the
+    order of application equals the printed order.  With a potential the caller supplies the
+    phase planes of the two distinct sub-steps: pot_p = (cos, -sin)(V p dt) and
+    pot_q = (cos, -sin)(V (1-4p) dt).
+    """
+    if (pot_p is None) != (pot_q is None):
+        raise ValueError("give both pot_p and pot_q or neither")
+    import math
+    for _ in range(int(n_steps)):
+        for k, f in enumerate(u4_fractions()):
+            th = f * theta
+            pot = None if pot_p is None else (pot_q if k == 2 else pot_p)
+            evolve(re, im, math.cos(th / 2), math.sin(th / 2), math.cos(th), math.sin(th),
+                   pot=pot, periodic=periodic, n_steps=1)
+
+
 def norm2(re, im) -> float:
     re = np.ascontiguousarray(re, dtype=np.float64)
     im = np.ascontiguousarray(im, dtype=np.float64)
