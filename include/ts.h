@@ -73,6 +73,26 @@ int ts_evolve(ts_plan* plan, void* psi_re, void* psi_im,
               const void* pot_phase_or_null, int64_t n_steps, void* cuda_stream);
 
 /*
+ * ts_evolve_u4 -- psi <- U4^n_steps psi, the fourth-order step of Eq. 4:
+ *
+ *      U4(dt) = U2(p dt) U2(p dt) U2((1-4p) dt) U2(p dt) U2(p dt),     p = (4 - 4^(1/3))^-1,
+ *
+ * every U2(f dt) being the second-order step of ts_evolve with angle f*theta (coefficients
+ * cos/sin(f theta/2), cos/sin(f theta), computed in double inside the library).
+ *   theta            full-step angle dt*|V_tunnel|/hbar in radians, finite; its sign is the caller's.
+ *   pot_phase_p_or_null, pot_phase_q_or_null
+ *                    both NULL (no potential) or both DEVICE pointers to 2*ny*nx elements laid out
+ *                    like pot_phase of ts_evolve: the phases of the two distinct sub-steps,
+ *                    exp(-i V p dt) and exp(-i V (1-4p) dt).
+ * Other arguments, asynchrony, scratch use and errors as for ts_evolve.  The five sub-steps are
+ * chained inside the fused kernel like ordinary steps (per-sub-step angle table), so a
+ * fourth-order step costs five second-order sub-steps, not five passes over HBM.
+ */
+int ts_evolve_u4(ts_plan* plan, void* psi_re, void* psi_im, double theta,
+                 const void* pot_phase_p_or_null, const void* pot_phase_q_or_null,
+                 int64_t n_steps, void* cuda_stream);
+
+/*
  * ts_norm -- squared norm sum |psi|^2, accumulated in double for either dtype.
  *   psi_re, psi_im   DEVICE pointers as above (read only).
  *   out_norm2_host   HOST pointer to one double, written before the call returns.

@@ -13,7 +13,7 @@ TS_MAX_FUSE = 6
 _LIB_PATH = Path(__file__).resolve().parent / "libts.so"
 _lib = None
 
-SYMBOLS = ["ts_plan_create", "ts_evolve", "ts_norm", "ts_evolve_host", "ts_plan_set_option",
+SYMBOLS = ["ts_plan_create", "ts_evolve", "ts_evolve_u4", "ts_norm", "ts_evolve_host", "ts_plan_set_option",
            "ts_plan_get_info", "ts_plan_destroy", "ts_last_error"]
 
 
@@ -36,6 +36,8 @@ def lib():
         L.ts_plan_create.restype = vp
         L.ts_evolve.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp, i64, vp]
         L.ts_evolve.restype = i32
+        L.ts_evolve_u4.argtypes = [vp, vp, vp, dbl, vp, vp, i64, vp]
+        L.ts_evolve_u4.restype = i32
         L.ts_norm.argtypes = [vp, vp, vp, ctypes.POINTER(dbl), vp]
         L.ts_norm.restype = i32
         L.ts_evolve_host.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp, i64]
@@ -119,6 +121,25 @@ class Plan:
         _check(lib().ts_evolve(self._h, ctypes.c_void_p(psi_re.data_ptr()),
                                ctypes.c_void_p(psi_im.data_ptr()), a_half, b_half, a_full, b_full,
                                pot, int(n_steps), _stream_handle(stream)))
+
+    def _pot_ptr(self, pot_phase):
+        if pot_phase is None:
+            return None
+        if pot_phase.dtype != self.dtype or tuple(pot_phase.shape) != (2, self.ny, self.nx) \
+                or not pot_phase.is_contiguous() or not pot_phase.is_cuda:
+            raise ValueError("pot_phase must be a contiguous CUDA tensor [2][ny][nx]")
+        return ctypes.c_void_p(pot_phase.data_ptr())
+
+    def evolve_u4(self, psi_re, psi_im, theta, pot_phase_p=None, pot_phase_q=None, n_steps=1,
+                  stream=None):
+        """ts_evolve_u4 (fourth-order step, Eq. 4) on CUDA tensors, in place, asynchronous."""
+        self._planes(psi_re, psi_im)
+        if not (psi_re.is_cuda and psi_im.is_cuda):
+            raise ValueError("evolve_u4 takes CUDA tensors")
+        _check(lib().ts_evolve_u4(self._h, ctypes.c_void_p(psi_re.data_ptr()),
+                                  ctypes.c_void_p(psi_im.data_ptr()), float(theta),
+                                  self._pot_ptr(pot_phase_p), self._pot_ptr(pot_phase_q),
+                                  int(n_steps), _stream_handle(stream)))
 
     def evolve_host(self, psi_re, psi_im, a_half, b_half, a_full, b_full, pot_phase=None,
                     n_steps=1):

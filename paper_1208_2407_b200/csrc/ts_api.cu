@@ -161,48 +161,81 @@ int ts_plan_get_info(const ts_plan* plan, const char* name, int64_t* out) {
     return TS_OK;
 }
 
-int ts_evolve(ts_plan* plan, void* psi_re, void* psi_im, double a_half, double b_half,
-              double a_full, double b_full, const void* pot, int64_t n_steps, void* cuda_stream) {
+}  // extern "C"
+
+namespace {
+
+struct SubStep {
+    ts::StepCoef c;
+    const void* pot;   // device phase planes of this sub-step or nullptr
+};
+
+// psi <- (U2(pat[P-1]) ... U2(pat[0]))^n_repeat psi: the engine behind ts_evolve (P = 1) and
+// ts_evolve_u4 (P = 5).  Consecutive sub-steps that share a potential-phase array are fused into
+// passes of up to S sub-steps; passes ping-pong between the caller's planes and the scratch.
+int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat, int period,
+                   int64_t n_repeat, void* cuda_stream) {
     if (!plan) return fail(TS_EINVAL, "NULL plan");
     if (!psi_re || !psi_im) return fail(TS_EINVAL, "NULL psi plane");
-    if (n_steps < 0) return fail(TS_EINVAL, "n_steps < 0");
-    if (!coef_ok(a_half, b_half) || !coef_ok(a_full, b_full))
-        return fail(TS_EINVAL, "coefficients must be finite with |a^2 + b^2 - 1| <= 1e-6");
+    if (n_repeat < 0) return fail(TS_EINVAL, "n_steps < 0");
     const ts::LatticeDesc& L = plan->L;
     const size_t plane_bytes = (size_t)L.nx * (size_t)L.ny * plan->elem;
-    if (!aligned16(psi_re) || !aligned16(psi_im) || (pot && !aligned16(pot)))
+    if (!aligned16(psi_re) || !aligned16(psi_im))
         return fail(TS_EINVAL, "device pointers must be 16-byte aligned");
     if (overlap(psi_re, psi_im, plane_bytes)) return fail(TS_EINVAL, "psi_re and psi_im overlap");
-    if (pot && (overlap(pot, psi_re, plane_bytes) || overlap(pot, psi_im, plane_bytes) ||
+    bool any_pot = false, can_fuse = true, can_stream = true;
+    for (int k = 0; k < period; ++k) {
+        const ts::StepCoef& c = pat[k].c;
+        if (!coef_ok(c.a_h, c.b_h) || !coef_ok(c.a_f, c.b_f))
+            return fail(TS_EINVAL, "coefficients must be finite with |a^2 + b^2 - 1| <= 1e-6");
+        const void* pot = pat[k].pot;
+        if (pot) {
+            any_pot = true;
+            if (!aligned16(pot)) return fail(TS_EINVAL, "device pointers must be 16-byte aligned");
+            if (overlap(pot, psi_re, plane_bytes) || overlap(pot, psi_im, plane_bytes) ||
                 overlap((const char*)pot + plane_bytes, psi_re, plane_bytes) ||
-                overlap((const char*)pot + plane_bytes, psi_im, plane_bytes)))
-        return fail(TS_EINVAL, "pot_phase overlaps psi");
+                overlap((const char*)pot + plane_bytes, psi_im, plane_bytes))
+                return fail(TS_EINVAL, "pot_phase overlaps psi");
+        }
+        can_fuse = can_fuse && ts::fused_supported(L, c);
+        can_stream = can_stream && ts::stream_supported(L, c);
+    }
     int rc = check_device(plan);
     if (rc != TS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
 
     plan->info_fused = plan->info_fuse = plan->info_passes = plan->info_launches = 0;
     plan->info_seg = plan->info_variant = 0;
-    if (n_steps == 0) return TS_OK;
+    if (n_repeat == 0) return TS_OK;
+    if (period > 1 && n_repeat > (int64_t(1) << 56)) return fail(TS_EINVAL, "n_steps too large");
+    const int64_t n_sub = n_repeat * period;
 
-    const ts::StepCoef c{a_half, b_half, a_full, b_full};
-    const bool can_fuse = ts::fused_supported(L, c);
     if (plan->opt_path == 2 && !can_fuse)
         return fail(TS_EUNSUPPORTED,
                     "fused kernel needs nx % 4 == 0, even ny and cos(theta) > 0.25");
-    if (plan->opt_path == 1 || !can_fuse)
-        return ts::generic_evolve(L, psi_re, psi_im, c, pot, n_steps, st, &plan->info_launches);
+    if (plan->opt_path == 1 || !can_fuse) {
+        if (period == 1)
+            return ts::generic_evolve(L, psi_re, psi_im, pat[0].c, pat[0].pot, n_repeat, st,
+                                      &plan->info_launches);
+        for (int64_t i = 0; i < n_sub; ++i) {
+            const SubStep& s = pat[i % period];
+            int64_t launches = 0;
+            rc = ts::generic_evolve(L, psi_re, psi_im, s.c, s.pot, 1, st, &launches);
+            if (rc != TS_OK) return rc;
+            plan->info_launches += launches;
+        }
+        return TS_OK;
+    }
 
     rc = ensure_alloc(&plan->scratch_re, plane_bytes);
     if (rc == TS_OK) rc = ensure_alloc(&plan->scratch_im, plane_bytes);
     if (rc != TS_OK) return rc;
 
-    const bool can_stream = ts::stream_supported(L, c);
     if (plan->opt_variant == 2 && !can_stream)
         return fail(TS_EUNSUPPORTED, "the TMA ring kernel needs nx >= 128");
     const bool use_stream = can_stream && plan->opt_variant != 1;
-    int S = plan->opt_fuse ? (int)plan->opt_fuse : ts::fused_default_steps(L, pot != nullptr);
-    const int s_max = use_stream ? ts::stream_max_steps(L, pot != nullptr) : 4;
+    int S = plan->opt_fuse ? (int)plan->opt_fuse : ts::fused_default_steps(L, any_pot);
+    const int s_max = use_stream ? ts::stream_max_steps(L, any_pot) : 4;
     if (S > s_max) {
         if (plan->opt_fuse)
             return fail(TS_EUNSUPPORTED, "fuse_steps > 4 needs the TMA ring kernel, fp32, no potential");
@@ -212,19 +245,29 @@ int ts_evolve(ts_plan* plan, void* psi_re, void* psi_im, double a_half, double b
     plan->info_variant = use_stream ? 2 : 1;
     void* cur_re = psi_re; void* cur_im = psi_im;
     void* nxt_re = plan->scratch_re; void* nxt_im = plan->scratch_im;
-    int64_t left = n_steps;
-    while (left > 0) {
-        const int s = left >= S ? S : (int)left;
+    int64_t i = 0;
+    while (i < n_sub) {
+        // the run of sub-steps of this pass: same potential array; the register-prefetch kernel
+        // (variant 1) also needs equal angles
+        ts::StepCoef subs[TS_MAX_FUSE];
+        const void* pot = pat[i % period].pot;
+        int s = 0;
+        while (s < S && i + s < n_sub) {
+            const SubStep& x = pat[(i + s) % period];
+            if (x.pot != pot) break;
+            if (!use_stream && s > 0 && memcmp(&x.c, &subs[0], sizeof(ts::StepCoef)) != 0) break;
+            subs[s++] = x.c;
+        }
         if (use_stream)
-            rc = ts::stream_pass(L, cur_re, cur_im, nxt_re, nxt_im, c, pot, s, seg,
+            rc = ts::stream_pass(L, cur_re, cur_im, nxt_re, nxt_im, subs, pot, s, seg,
                                  (int)plan->opt_slots, st);
         else
-            rc = ts::fused_pass(L, cur_re, cur_im, nxt_re, nxt_im, c, pot, s, seg, st);
+            rc = ts::fused_pass(L, cur_re, cur_im, nxt_re, nxt_im, subs[0], pot, s, seg, st);
         if (rc != TS_OK) return rc;
         void* t;
         t = cur_re; cur_re = nxt_re; nxt_re = t;
         t = cur_im; cur_im = nxt_im; nxt_im = t;
-        left -= s;
+        i += s;
         ++plan->info_passes;
         ++plan->info_launches;
     }
@@ -237,6 +280,33 @@ int ts_evolve(ts_plan* plan, void* psi_re, void* psi_im, double a_half, double b
     plan->info_fuse = S;
     plan->info_seg = seg;
     return TS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ts_evolve(ts_plan* plan, void* psi_re, void* psi_im, double a_half, double b_half,
+              double a_full, double b_full, const void* pot, int64_t n_steps, void* cuda_stream) {
+    const SubStep one{{a_half, b_half, a_full, b_full}, pot};
+    return evolve_pattern(plan, psi_re, psi_im, &one, 1, n_steps, cuda_stream);
+}
+
+int ts_evolve_u4(ts_plan* plan, void* psi_re, void* psi_im, double theta, const void* pot_p,
+                 const void* pot_q, int64_t n_steps, void* cuda_stream) {
+    if ((pot_p == nullptr) != (pot_q == nullptr))
+        return fail(TS_EINVAL, "give both potential-phase arrays of the fourth-order step or neither");
+    if (!isfinite(theta)) return fail(TS_EINVAL, "theta must be finite");
+    // Eq. 4: U4(dt) = U2(p dt) U2(p dt) U2((1-4p) dt) U2(p dt) U2(p dt)
+    const double p = 1.0 / (4.0 - cbrt(4.0));
+    const double frac[5] = {p, p, 1.0 - 4.0 * p, p, p};
+    SubStep pat[5];
+    for (int k = 0; k < 5; ++k) {
+        const double th = frac[k] * theta;
+        pat[k].c = ts::StepCoef{cos(0.5 * th), sin(0.5 * th), cos(th), sin(th)};
+        pat[k].pot = k == 2 ? pot_q : pot_p;
+    }
+    return evolve_pattern(plan, psi_re, psi_im, pat, 5, n_steps, cuda_stream);
 }
 
 int ts_norm(ts_plan* plan, const void* psi_re, const void* psi_im, double* out, void* cuda_stream) {

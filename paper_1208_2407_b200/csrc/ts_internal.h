@@ -50,8 +50,10 @@ int fused_default_seg_rows(const LatticeDesc& L, int S);
 bool stream_supported(const LatticeDesc& L, const StepCoef& c);
 int stream_max_steps(const LatticeDesc& L, bool pot);   // 6 for fp32 without potential, else 4
 int stream_default_slots(const LatticeDesc& L, int S, bool pot);
+// One pass: dst <- U2(subs[S-1]) ... U2(subs[0]) src; the S sub-steps may have different angles
+// (fourth-order step, Eq. 4) but share one potential-phase array.
 int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
-                void* dst_im, const StepCoef& c, const void* pot, int S, int seg_rows, int nst,
+                void* dst_im, const StepCoef* subs, const void* pot, int S, int seg_rows, int nst,
                 cudaStream_t st);
 int fused_default_steps(const LatticeDesc& L, bool pot);
 

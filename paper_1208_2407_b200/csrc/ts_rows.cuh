@@ -145,6 +145,25 @@ __device__ __forceinline__ void xo(Row4<T>& r, T t, const XEdge<T>& e) {
     }
 }
 
+// The same with the coupling given per call (the angle may change from sub-step to sub-step):
+// the lane only remembers WHERE its cross-lane pairs are cut by a closed edge.
+struct XCut {
+    bool up;   // pair (site 0, previous lane's site 3) straddles a closed edge (or is all ghost)
+    bool dn;   // pair (site 3, next lane's site 0) does
+};
+template <typename T, bool EDGE>
+__device__ __forceinline__ void xo(Row4<T>& r, T t, T sec, const XCut& m) {
+    if (EDGE) {
+        XEdge<T> e;
+        e.t_up = m.up ? T(0) : t;  e.c0 = m.up ? sec : T(1);
+        e.t_dn = m.dn ? T(0) : t;  e.c3 = m.dn ? sec : T(1);
+        xo<T, true>(r, t, e);
+    } else {
+        XEdge<T> e;   // unused by the plain form
+        xo<T, false>(r, t, e);
+    }
+}
+
 // vertical pair sweep between two rows held by the same lane
 template <typename T>
 __device__ __forceinline__ void ypair(Row4<T>& a, Row4<T>& b, T t) {

@@ -39,7 +39,13 @@ struct StreamParams {
     int nx, ny;
     int n_strips, wi, halo, seg_rows;
     int nst;        // ring slots per warp
-    T t_h, t_f, sec_h, sec_f, out_scale;
+    // tangents of the sweeps of the S chained sub-steps of this pass (angles may differ from
+    // sub-step to sub-step: Eq. 4 chains U2 with three different time fractions)
+    T te[TS_MAX_FUSE + 1];   // even sweeps: te[0] opening half sweep, te[j] the merged sweep between
+                             // sub-steps j-1 and j (half + half angle), te[S] the closing half sweep
+    T to[TS_MAX_FUSE];       // odd sweeps of sub-step j: full angle without potential, half with
+    T sec_o[TS_MAX_FUSE];    // 1 / cos of that odd sweep (unpaired sites at closed edges)
+    T out_scale;             // product of all deferred cosines of the pass
 };
 
 // ---- PTX: mbarrier + bulk async copy (TMA) -------------------------------------------------------
@@ -105,33 +111,33 @@ template <typename T>
 struct StreamCtx {
     bool xvalid;         // lane's sites exist (always when periodic)
     bool xedge;          // warp-uniform: strip touches a closed edge in x
-    XEdge<T> e;
+    XCut e;              // where the lane's cross-lane X-odd pairs meet a closed edge
     uint32_t ring;       // shared address of the warp's slot ring
     uint32_t lane_off;   // byte offset of the lane's 4 sites inside a row chunk
 };
 
-// One second-order step of the register pipeline.
+// One second-order sub-step (stage J of S) of the register pipeline, WITH a potential.
 //   in : (a0, a1) = rows (yj, yj+1) before the step; (g, h) = rows (yj-2, yj-1) in mid-step state
 //   out: (g, h) = rows (yj-2, yj-1) after the step; (a0, a1) = rows (yj, yj+1) in mid-step state
-// FIRST / LAST: first / last step of the pass.  Between two chained steps the closing X-even
-// half sweep of one and the opening X-even half sweep of the next act on the same rows back to
-// back, Xe(h) Xe(h) = Xe(f), so an inner boundary applies ONE full-angle X-even sweep at the
-// start of the later step (the deferred cos factor is adjusted in out_scale).
+// Between two chained sub-steps the closing X-even half sweep of one and the opening X-even
+// half sweep of the next act on the same rows back to back and are applied as ONE sweep by the
+// sum of the two half angles (te[J]) at the start of the later sub-step; the deferred cosine
+// is accounted for in out_scale.
 // pot_yj / pot_yjm1: shared addresses of the potential rows yj (row 0 of its slot) and yj-1
-// (row 1 of the previous slot), valid when POT.
-template <typename T, bool POT, bool PER, bool XEDGE, bool FIRST, bool LAST>
+// (row 1 of the previous slot).
+template <typename T, bool PER, bool XEDGE, int S, int J>
 __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const StreamCtx<T>& c,
                                              int yj, Row4<T>& a0, Row4<T>& a1, Row4<T>& g,
                                              Row4<T>& h, uint32_t pot_yj, uint32_t pot_yjm1) {
     constexpr uint32_t ROWB = kStripSites * sizeof(T);
-    const T t_open = FIRST ? p.t_h : p.t_f;
-    xe(a0, t_open); xe(a1, t_open);
-    xo<T, XEDGE>(a0, p.t_h, c.e); xo<T, XEDGE>(a1, p.t_h, c.e);
-    ypair(a0, a1, p.t_h);
+    const T th = p.to[J];
+    xe(a0, p.te[J]); xe(a1, p.te[J]);
+    xo<T, XEDGE>(a0, th, p.sec_o[J], c.e); xo<T, XEDGE>(a1, th, p.sec_o[J], c.e);
+    ypair(a0, a1, th);
     // closed lattice: the vertical-odd pair (yj-1, yj) does not exist at yj = 0 and yj = ny; the
     // ghost row is zero and stays zero (coupling 0), the real row takes 1/a per omitted sweep
     const bool yedge = XEDGE && (yj == 0 || yj == p.ny);
-    const T t_yo = yedge ? T(0) : p.t_h;
+    const T t_yo = yedge ? T(0) : th;
     ypair(h, a0, t_yo);
     {
         const bool lo_ok = !XEDGE || (c.xvalid && yj - 1 >= 0 && yj - 1 < p.ny);
@@ -151,40 +157,68 @@ __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const Str
     }
     ypair(h, a0, t_yo);
     if (XEDGE) {
-        const T sy = yedge ? p.sec_h * p.sec_h : T(1);
+        const T sy = yedge ? p.sec_o[J] * p.sec_o[J] : T(1);
         scale_row(h, sy); scale_row(a0, sy);
     }
-    ypair(g, h, p.t_h);
-    xo<T, XEDGE>(g, p.t_h, c.e); xo<T, XEDGE>(h, p.t_h, c.e);
-    if (LAST) { xe(g, p.t_h); xe(h, p.t_h); }
+    ypair(g, h, th);
+    xo<T, XEDGE>(g, th, p.sec_o[J], c.e); xo<T, XEDGE>(h, th, p.sec_o[J], c.e);
+    if (J == S - 1) { xe(g, p.te[S]); xe(h, p.te[S]); }
 }
 
-// The same step WITHOUT a potential, regrouped.  Horizontal sweeps act inside a row and vertical
-// sweeps act along a column with the same scalar coefficients, so every X sweep commutes with every
-// Y sweep (tensor-product structure; pinned on the oracle by test_xy_regrouping and on dense
-// matrices by test_stage_order...).  The step Xe Xo Ye Yo(f) Ye Xo Xe therefore equals
-// [Xe(h) Xo(f) Xe(h)] [Ye(h) Yo(f) Ye(h)], and across chained steps the adjacent half sweeps merge:
-// per pass  X: Xe(h) Xo(f) {Xe(f) Xo(f)}^(S-1) Xe(h),  Y: likewise.  4S+2 sweeps instead of 7S.
-// Only the rounding differs from the literal sequence.
+// The same sub-step WITHOUT a potential, regrouped.  Horizontal sweeps act inside a row and
+// vertical sweeps act along a column with the same scalar coefficients, so every X sweep commutes
+// with every Y sweep (tensor-product structure; pinned on the oracle by test_xy_regrouping and on
+// dense matrices by test_stage_order...).  The step Xe Xo Ye Yo(f) Ye Xo Xe therefore equals
+// [Xe(h) Xo(f) Xe(h)] [Ye(h) Yo(f) Ye(h)], and across chained sub-steps the adjacent half sweeps
+// merge: per pass  X: Xe(h0) Xo(f0) {Xe(h_{j-1} + h_j) Xo(f_j)}_{j=1..S-1} Xe(h_{S-1}),  Y: likewise.
+// 4S+2 sweeps instead of 7S.  Only the rounding differs from the literal sequence.
 //   in : (a0, a1) = rows (yj, yj+1) entering step; (g, h) = rows (yj-2, yj-1), h waiting for Yo
 //   out: (g, h) finished with this step; (a0, a1) held for the next iteration
-template <typename T, bool PER, bool XEDGE, bool FIRST, bool LAST>
+template <typename T, bool PER, bool XEDGE, int S, int J>
 __device__ __forceinline__ void stream_stage_nopot(const StreamParams<T>& p,
                                                    const StreamCtx<T>& c, int yj, Row4<T>& a0,
                                                    Row4<T>& a1, Row4<T>& g, Row4<T>& h) {
-    const T t_open = FIRST ? p.t_h : p.t_f;
-    xe(a0, t_open); xe(a1, t_open);
-    xo<T, XEDGE>(a0, p.t_f, c.e); xo<T, XEDGE>(a1, p.t_f, c.e);
-    if (LAST) { xe(a0, p.t_h); xe(a1, p.t_h); }
-    ypair(a0, a1, t_open);
+    constexpr bool LAST = J == S - 1;
+    xe(a0, p.te[J]); xe(a1, p.te[J]);
+    xo<T, XEDGE>(a0, p.to[J], p.sec_o[J], c.e); xo<T, XEDGE>(a1, p.to[J], p.sec_o[J], c.e);
+    if (LAST) { xe(a0, p.te[S]); xe(a1, p.te[S]); }
+    ypair(a0, a1, p.te[J]);
     // closed lattice: the vertical-odd pair (yj-1, yj) does not exist at yj = 0 and yj = ny; the
     // real row of the two takes 1/a instead (the ghost row is zero and stays zero)
     const bool yedge = XEDGE && (yj == 0 || yj == p.ny);
-    const T t_yo = yedge ? T(0) : p.t_f;
+    const T t_yo = yedge ? T(0) : p.to[J];
     ypair(h, a0, t_yo);
-    if (XEDGE) { const T sy = yedge ? p.sec_f : T(1); scale_row(h, sy); scale_row(a0, sy); }
-    if (LAST) ypair(g, h, p.t_h);
+    if (XEDGE) { const T sy = yedge ? p.sec_o[J] : T(1); scale_row(h, sy); scale_row(a0, sy); }
+    if (LAST) ypair(g, h, p.te[S]);
 }
+
+// stages 0..S-1 of one iteration: the pair (x0, x1) flows through them, see the kernel
+template <typename T, bool POT, bool PER, bool XEDGE, int S, int J>
+struct Stages {
+    static __device__ __forceinline__ void run(const StreamParams<T>& p, const StreamCtx<T>& c,
+                                               int y, int cs, int nst, uint32_t slotb,
+                                               Row4<T> (&W)[S][2][2], const int u, Row4<T>& x0,
+                                               Row4<T>& x1) {
+        constexpr uint32_t ROWB = kStripSites * sizeof(T);
+        Row4<T>& a0 = W[J][u][0];
+        Row4<T>& a1 = W[J][u][1];
+        Row4<T>& g = W[J][u ^ 1][0];
+        Row4<T>& h = W[J][u ^ 1][1];
+        a0 = x0; a1 = x1;
+        if (POT) {
+            int s0 = cs - J;      if (s0 < 0) s0 += nst;
+            int s1 = s0 - 1;      if (s1 < 0) s1 += nst;
+            const uint32_t pot_yj = c.ring + s0 * slotb + 4 * ROWB;
+            const uint32_t pot_yjm1 = c.ring + s1 * slotb + 6 * ROWB;
+            stream_stage<T, PER, XEDGE, S, J>(p, c, y - 2 * J, a0, a1, g, h, pot_yj, pot_yjm1);
+        } else {
+            stream_stage_nopot<T, PER, XEDGE, S, J>(p, c, y - 2 * J, a0, a1, g, h);
+        }
+        x0 = g; x1 = h;   // (g, h) left the sub-step and flows on; (a0, a1) now waits in stage J
+        if constexpr (J + 1 < S)
+            Stages<T, POT, PER, XEDGE, S, J + 1>::run(p, c, y, cs, nst, slotb, W, u, x0, x1);
+    }
+};
 
 template <typename T, int S, bool POT, bool PER, int MINB>
 __global__ void __launch_bounds__(kWarps * 32, MINB)
@@ -208,12 +242,8 @@ stream_kernel(const StreamParams<T> p) {
     StreamCtx<T> c;
     c.xvalid = PER ? true : (xb >= 0 && xb < p.nx);
     c.xedge = !PER && (xs < 0 || xs + kStripSites > p.nx);
-    const T t_xo = POT ? p.t_h : p.t_f;       // X-odd sweeps are full-angle when regrouped
-    const T sec_xo = POT ? p.sec_h : p.sec_f;
-    c.e.t_up = (xb == 0 || xb == p.nx) ? T(0) : t_xo;
-    c.e.t_dn = (xb + 4 == p.nx || xb + 4 == 0) ? T(0) : t_xo;
-    c.e.c0 = (xb == 0) ? sec_xo : T(1);
-    c.e.c3 = (xb + 4 == p.nx) ? sec_xo : T(1);
+    c.e.up = !PER && (xb == 0 || xb == p.nx);
+    c.e.dn = !PER && (xb + 4 == p.nx || xb + 4 == 0);
     c.ring = smem_u32(smem_raw) + warp * NST * SLOTB;
     c.lane_off = lane * 4 * sizeof(T);
     const uint32_t bars = smem_u32(smem_raw) + kWarps * NST * SLOTB + warp * NST * 8;
@@ -310,9 +340,9 @@ stream_kernel(const StreamParams<T> p) {
 
 #pragma unroll 1
     for (int it0 = 0; it0 < n_iter; it0 += 2) {
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            const int it = it0 + u;
+        auto half = [&](auto utag) {
+            constexpr int U = decltype(utag)::value;
+            const int it = it0 + U;
             {
                 __syncwarp();   // every lane is done with the slot about to be refilled
                 if (it + DIST < n_iter) issue(rs);
@@ -330,41 +360,7 @@ stream_kernel(const StreamParams<T> p) {
                     zero_row(x0);
                     zero_row(x1);
                 }
-#pragma unroll
-                for (int j = 0; j < S; ++j) {
-                    uint32_t pot_yj = 0, pot_yjm1 = 0;
-                    if (POT) {
-                        int s0 = cs - j;      if (s0 < 0) s0 += NST;
-                        int s1 = s0 - 1;      if (s1 < 0) s1 += NST;
-                        pot_yj = c.ring + s0 * SLOTB + 4 * ROWB;
-                        pot_yjm1 = c.ring + s1 * SLOTB + 6 * ROWB;
-                    }
-                    Row4<T>& a0 = W[j][u][0];
-                    Row4<T>& a1 = W[j][u][1];
-                    Row4<T>& g = W[j][u ^ 1][0];
-                    Row4<T>& h = W[j][u ^ 1][1];
-                    a0 = x0; a1 = x1;
-                    if (POT) {
-                        if (j == 0 && j == S - 1)
-                            stream_stage<T, POT, PER, XEDGE, true, true>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
-                        else if (j == 0)
-                            stream_stage<T, POT, PER, XEDGE, true, false>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
-                        else if (j == S - 1)
-                            stream_stage<T, POT, PER, XEDGE, false, true>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
-                        else
-                            stream_stage<T, POT, PER, XEDGE, false, false>(p, c, y - 2 * j, a0, a1, g, h, pot_yj, pot_yjm1);
-                    } else {
-                        if (j == 0 && j == S - 1)
-                            stream_stage_nopot<T, PER, XEDGE, true, true>(p, c, y - 2 * j, a0, a1, g, h);
-                        else if (j == 0)
-                            stream_stage_nopot<T, PER, XEDGE, true, false>(p, c, y - 2 * j, a0, a1, g, h);
-                        else if (j == S - 1)
-                            stream_stage_nopot<T, PER, XEDGE, false, true>(p, c, y - 2 * j, a0, a1, g, h);
-                        else
-                            stream_stage_nopot<T, PER, XEDGE, false, false>(p, c, y - 2 * j, a0, a1, g, h);
-                    }
-                    x0 = g; x1 = h;
-                }
+                Stages<T, POT, PER, XEDGE, S, 0>::run(p, c, y, cs, NST, SLOTB, W, U, x0, x1);
                 if (it >= 2 * S && store_ok && y - 2 * S < y_out1) {
                     const int64_t off = (int64_t)(y - 2 * S) * p.nx + xb;
                     st4(p.dst_re + off, x0.re, p.out_scale);
@@ -375,7 +371,9 @@ stream_kernel(const StreamParams<T> p) {
                 if (++cs == NST) { cs = 0; cph ^= 1; }
                 if (++rs == NST) rs = 0;
             }
-        }
+        };
+        half(std::integral_constant<int, 0>{});
+        half(std::integral_constant<int, 1>{});
     }
     };   // run
     const bool edge = !PER && (c.xedge || y_in0 < 0 || y_in0 + 2 * n_iter >= p.ny);
@@ -415,7 +413,7 @@ int launch_s(const StreamParams<T>& p, bool pot, bool per, cudaStream_t st) {
 
 template <typename T>
 int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T* dst_im,
-           const StepCoef& c, const T* pot, int S, int seg_rows, int nst, cudaStream_t st) {
+           const StepCoef* subs, const T* pot, int S, int seg_rows, int nst, cudaStream_t st) {
     StreamParams<T> p;
     p.src_re = src_re; p.src_im = src_im; p.dst_re = dst_re; p.dst_im = dst_im;
     p.pot_re = pot;
@@ -431,18 +429,42 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
     const size_t slotb = (size_t)(pot ? 8 : 4) * kStripSites * sizeof(T);
     while (nst > live + 1 && (size_t)kWarps * nst * (slotb + 8) > 227u * 1024u) --nst;
     p.nst = nst;
-    p.t_h = (T)(c.b_h / c.a_h);
-    p.t_f = (T)(c.b_f / c.a_f);
-    p.sec_h = (T)(1.0 / c.a_h);
-    p.sec_f = (T)(1.0 / c.a_f);
-    const double per_step = pot ? pow(c.a_h, 8) : pow(c.a_h, 6) * c.a_f;
-    if (pot) {
-        // each of the S-1 inner step boundaries applies one Xe(f) instead of Xe(h) Xe(h)
-        p.out_scale = (T)(pow(per_step, S) * pow(c.a_f / (c.a_h * c.a_h), S - 1));
-    } else {
-        // regrouped: per axis Xe(h), S x Xo(f), (S-1) x Xe(f), Xe(h)
-        p.out_scale = (T)(pow(c.a_h, 4) * pow(c.a_f, 4 * S - 2));
+    // tangents and deferred cosines of the S sub-steps (all in double, rounded once).  The merged
+    // even sweep between sub-steps j-1 and j rotates by the sum of their half angles:
+    // cos = a a' - b b', sin = a b' + b a'.
+    double scale = 1.0;
+    {
+        const StepCoef& f = subs[0];
+        const StepCoef& l = subs[S - 1];
+        p.te[0] = (T)(f.b_h / f.a_h);
+        p.te[S] = (T)(l.b_h / l.a_h);
+        const double ends = f.a_h * l.a_h;
+        scale *= pot ? ends : ends * ends;           // X only, or X and Y (regrouped)
     }
+    for (int j = 1; j < S; ++j) {
+        const StepCoef& u = subs[j - 1];
+        const StepCoef& v = subs[j];
+        const double cm = u.a_h * v.a_h - u.b_h * v.b_h;
+        const double sm = u.a_h * v.b_h + u.b_h * v.a_h;
+        p.te[j] = (T)(sm / cm);
+        scale *= pot ? cm : cm * cm;
+    }
+    for (int j = 0; j < S; ++j) {
+        const StepCoef& v = subs[j];
+        if (pot) {
+            // Xo, Ye, Yo at the half angle, each twice per sub-step
+            p.to[j] = (T)(v.b_h / v.a_h);
+            p.sec_o[j] = (T)(1.0 / v.a_h);
+            scale *= pow(v.a_h, 6);
+        } else {
+            // Xo and Yo at the full angle, once each
+            p.to[j] = (T)(v.b_f / v.a_f);
+            p.sec_o[j] = (T)(1.0 / v.a_f);
+            scale *= v.a_f * v.a_f;
+        }
+    }
+    for (int j = S; j < TS_MAX_FUSE; ++j) { p.to[j] = T(0); p.sec_o[j] = T(1); p.te[j + 1] = T(0); }
+    p.out_scale = (T)scale;
     const bool per = L.periodic != 0;
     switch (S) {
         case 1: return launch_s<T, 1>(p, pot != nullptr, per, st);
@@ -481,7 +503,7 @@ int stream_default_slots(const LatticeDesc& L, int S, bool pot) {
 }
 
 int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
-                void* dst_im, const StepCoef& c, const void* pot, int S, int seg_rows, int nst,
+                void* dst_im, const StepCoef* subs, const void* pot, int S, int seg_rows, int nst,
                 cudaStream_t st) {
     if (seg_rows <= 0 || seg_rows % 2) {
         set_error("stream_pass: seg_rows must be positive and even");
@@ -489,9 +511,9 @@ int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, vo
     }
     if (L.dtype == TS_F32)
         return pass_t<float>(L, (const float*)src_re, (const float*)src_im, (float*)dst_re,
-                             (float*)dst_im, c, (const float*)pot, S, seg_rows, nst, st);
+                             (float*)dst_im, subs, (const float*)pot, S, seg_rows, nst, st);
     return pass_t<double>(L, (const double*)src_re, (const double*)src_im, (double*)dst_re,
-                          (double*)dst_im, c, (const double*)pot, S, seg_rows, nst, st);
+                          (double*)dst_im, subs, (const double*)pot, S, seg_rows, nst, st);
 }
 
 }  // namespace ts

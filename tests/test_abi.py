@@ -16,7 +16,7 @@ HEADER = ROOT / "include" / "ts.h"
 
 def declared_functions():
     txt = re.sub(r"/\*.*?\*/", "", HEADER.read_text(), flags=re.S)
-    return sorted(set(re.findall(r"\b(ts_[a-z_]+)\s*\(", txt)))
+    return sorted(set(re.findall(r"\b(ts_[a-z0-9_]+)\s*\(", txt)))
 
 
 @pytest.fixture(scope="module")
