@@ -53,6 +53,15 @@ enum { TS_OK = 0, TS_EINVAL = 1, TS_EUNSUPPORTED = 2, TS_EALLOC = 3, TS_ECUDA = 
 ts_plan* ts_plan_create(int64_t nx, int64_t ny, int dtype, int boundary);
 
 /*
+ * ts_plan_create_xy -- the same with one boundary type per axis.  (TS_PERIODIC, TS_CLOSED) is what
+ * a row slab of a larger periodic lattice needs (domain decomposition: the
+ * slab plus its halo rows is evolved as a lattice that is closed in y; the rows within 2 sites per
+ * step of a cut are then wrong and are the halo that the next exchange overwrites).
+ * (TS_CLOSED, TS_PERIODIC) runs on the per-sweep kernels only.
+ */
+ts_plan* ts_plan_create_xy(int64_t nx, int64_t ny, int dtype, int boundary_x, int boundary_y);
+
+/*
  * ts_evolve -- psi <- U2^n_steps psi, in place from the caller's view (Eq. 3).
  *   psi_re, psi_im   DEVICE pointers, ny*nx elements each, 16-byte aligned, caller-owned.
  *   a_half, b_half   cos, sin of theta/2, theta = dt*|V_tunnel|/hbar.

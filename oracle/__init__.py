@@ -114,6 +114,30 @@ def evolve(re, im, a_half, b_half, a_full, b_full, pot=None, periodic=False, n_s
                           _ptr(pr), _ptr(pi), int(bool(periodic)), int(n_steps))
 
 
+def evolve_xy(re, im, a_half, b_half, a_full, b_full, pot=None, periodic_x=False,
+              periodic_y=False, n_steps=1) -> None:
+    """In place: n_steps second-order steps with one boundary type PER AXIS.
+
+    The stage list of SURVEY.md 8(c) / ``oracle_step`` written out with the C sweep and phase
+    routines (each pinned on its own), so that the horizontal sweeps can wrap while the vertical
+    ones do not: the lattice a row slab of a domain decomposition is evolved on.
+    """
+    _plane(re), _plane(im)
+    for _ in range(int(n_steps)):
+        sweep(re, im, 0, 0, a_half, b_half, periodic_x)
+        sweep(re, im, 0, 1, a_half, b_half, periodic_x)
+        sweep(re, im, 1, 0, a_half, b_half, periodic_y)
+        if pot is None:
+            sweep(re, im, 1, 1, a_full, b_full, periodic_y)
+        else:
+            sweep(re, im, 1, 1, a_half, b_half, periodic_y)
+            phase(re, im, pot[0], pot[1])
+            sweep(re, im, 1, 1, a_half, b_half, periodic_y)
+        sweep(re, im, 1, 0, a_half, b_half, periodic_y)
+        sweep(re, im, 0, 1, a_half, b_half, periodic_x)
+        sweep(re, im, 0, 0, a_half, b_half, periodic_x)
+
+
 # p of Eq. 4 (PAPER.md:95-101): p = (4 - 4^(1/3))^-1
 U4_P = 1.0 / (4.0 - 4.0 ** (1.0 / 3.0))
 

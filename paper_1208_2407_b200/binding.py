@@ -13,7 +13,7 @@ TS_MAX_FUSE = 6
 _LIB_PATH = Path(__file__).resolve().parent / "libts.so"
 _lib = None
 
-SYMBOLS = ["ts_plan_create", "ts_evolve", "ts_evolve_u4", "ts_norm", "ts_evolve_host", "ts_plan_set_option",
+SYMBOLS = ["ts_plan_create", "ts_plan_create_xy", "ts_evolve", "ts_evolve_u4", "ts_norm", "ts_evolve_host", "ts_plan_set_option",
            "ts_plan_get_info", "ts_plan_destroy", "ts_last_error"]
 
 
@@ -34,6 +34,8 @@ def lib():
         vp, i64, dbl, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int
         L.ts_plan_create.argtypes = [i64, i64, i32, i32]
         L.ts_plan_create.restype = vp
+        L.ts_plan_create_xy.argtypes = [i64, i64, i32, i32, i32]
+        L.ts_plan_create_xy.restype = vp
         L.ts_evolve.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp, i64, vp]
         L.ts_evolve.restype = i32
         L.ts_evolve_u4.argtypes = [vp, vp, vp, dbl, vp, vp, i64, vp]
@@ -80,13 +82,19 @@ def _stream_handle(stream):
 
 
 class Plan:
-    """ts_plan_create / ts_plan_destroy.  boundary: "closed" or "periodic"."""
+    """ts_plan_create[_xy] / ts_plan_destroy.  boundary: "closed" or "periodic"; boundary_y
+    defaults to the same (a different one per axis goes through ts_plan_create_xy)."""
 
-    def __init__(self, nx: int, ny: int, dtype, boundary: str = "closed"):
+    def __init__(self, nx: int, ny: int, dtype, boundary: str = "closed", boundary_y: str = None):
         self.nx, self.ny = int(nx), int(ny)
         self.dtype = dtype
-        b = {"closed": TS_CLOSED, "periodic": TS_PERIODIC}[boundary]
-        self._h = lib().ts_plan_create(self.nx, self.ny, _dtype_code(dtype), b)
+        codes = {"closed": TS_CLOSED, "periodic": TS_PERIODIC}
+        b = codes[boundary]
+        if boundary_y is None:
+            self._h = lib().ts_plan_create(self.nx, self.ny, _dtype_code(dtype), b)
+        else:
+            self._h = lib().ts_plan_create_xy(self.nx, self.ny, _dtype_code(dtype), b,
+                                              codes[boundary_y])
         if not self._h:
             raise TsError(TS_EINVAL, last_error())
 

@@ -86,18 +86,23 @@ extern "C" {
 const char* ts_last_error(void) { return ts::g_last_error.c_str(); }
 
 ts_plan* ts_plan_create(int64_t nx, int64_t ny, int dtype, int boundary) {
+    return ts_plan_create_xy(nx, ny, dtype, boundary, boundary);
+}
+
+ts_plan* ts_plan_create_xy(int64_t nx, int64_t ny, int dtype, int boundary, int boundary_y) {
     if (nx < 1 || ny < 1) { set_error("nx and ny must be >= 1"); return nullptr; }
     if (nx > (int64_t(1) << 31) || ny > (int64_t(1) << 31) || nx * ny >= (int64_t(1) << 62) / 16) {
         set_error("lattice too large");
         return nullptr;
     }
     if (dtype != TS_F32 && dtype != TS_F64) { set_error("unknown dtype"); return nullptr; }
-    if (boundary != TS_CLOSED && boundary != TS_PERIODIC) {
+    if ((boundary != TS_CLOSED && boundary != TS_PERIODIC) ||
+        (boundary_y != TS_CLOSED && boundary_y != TS_PERIODIC)) {
         set_error("unknown boundary");
         return nullptr;
     }
-    if (boundary == TS_PERIODIC && (nx % 2 || ny % 2)) {
-        set_error("periodic boundaries need even nx and ny (an odd ring cannot be split into "
+    if ((boundary == TS_PERIODIC && nx % 2) || (boundary_y == TS_PERIODIC && ny % 2)) {
+        set_error("a periodic axis needs an even extent (an odd ring cannot be split into "
                   "disjoint pairs)");
         return nullptr;
     }
@@ -107,7 +112,7 @@ ts_plan* ts_plan_create(int64_t nx, int64_t ny, int dtype, int boundary) {
     ts_plan* p = new (std::nothrow) ts_plan();
     if (!p) { set_error("out of host memory"); return nullptr; }
     memset(p, 0, sizeof(*p));
-    p->L.nx = nx; p->L.ny = ny; p->L.dtype = dtype; p->L.periodic = boundary == TS_PERIODIC;
+    p->L.nx = nx; p->L.ny = ny; p->L.dtype = dtype; p->L.periodic_x = boundary == TS_PERIODIC; p->L.periodic_y = boundary_y == TS_PERIODIC;
     p->device = dev;
     p->elem = dtype == TS_F32 ? 4 : 8;
     return p;
@@ -183,7 +188,7 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
     if (!aligned16(psi_re) || !aligned16(psi_im))
         return fail(TS_EINVAL, "device pointers must be 16-byte aligned");
     if (overlap(psi_re, psi_im, plane_bytes)) return fail(TS_EINVAL, "psi_re and psi_im overlap");
-    bool any_pot = false, can_fuse = true, can_stream = true;
+    bool any_pot = false, can_v1 = true, can_stream = true;
     for (int k = 0; k < period; ++k) {
         const ts::StepCoef& c = pat[k].c;
         if (!coef_ok(c.a_h, c.b_h) || !coef_ok(c.a_f, c.b_f))
@@ -197,9 +202,10 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
                 overlap((const char*)pot + plane_bytes, psi_im, plane_bytes))
                 return fail(TS_EINVAL, "pot_phase overlaps psi");
         }
-        can_fuse = can_fuse && ts::fused_supported(L, c);
+        can_v1 = can_v1 && ts::fused_supported(L, c);
         can_stream = can_stream && ts::stream_supported(L, c);
     }
+    const bool can_fuse = can_v1 || can_stream;
     int rc = check_device(plan);
     if (rc != TS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
@@ -233,6 +239,8 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
 
     if (plan->opt_variant == 2 && !can_stream)
         return fail(TS_EUNSUPPORTED, "the TMA ring kernel needs nx >= 128");
+    if (plan->opt_variant == 1 && !can_v1)
+        return fail(TS_EUNSUPPORTED, "the register-prefetch kernel needs one boundary type on both axes");
     const bool use_stream = can_stream && plan->opt_variant != 1;
     int S = plan->opt_fuse ? (int)plan->opt_fuse : ts::fused_default_steps(L, any_pot);
     const int s_max = use_stream ? ts::stream_max_steps(L, any_pot) : 4;

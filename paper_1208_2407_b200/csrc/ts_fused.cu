@@ -233,7 +233,7 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
     // deferred cos factors of one step: 6 half sweeps + the full one, or 8 half sweeps
     const double per_step = pot ? pow(c.a_h, 8) : pow(c.a_h, 6) * c.a_f;
     p.out_scale = (T)pow(per_step, S);
-    const bool per = L.periodic != 0;
+    const bool per = L.periodic_x != 0;
     switch (S) {
         case 1: return launch_s<T, 1>(p, pot != nullptr, per, st);
         case 2: return launch_s<T, 2>(p, pot != nullptr, per, st);
@@ -246,11 +246,15 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
 
 }  // namespace
 
-bool fused_supported(const LatticeDesc& L, const StepCoef& c) {
+bool fused_shape_ok(const LatticeDesc& L, const StepCoef& c) {
     // 128-bit row accesses need nx % 4 == 0; the row-pair pipeline needs even ny; the tangent
     // form needs cos well away from zero; 32-bit row/column indices inside the kernel.
     return L.nx % 4 == 0 && L.ny % 2 == 0 && L.nx >= 4 && L.ny >= 2 &&
            L.nx < (1 << 30) && L.ny < (1 << 30) && c.a_h > 0.25 && c.a_f > 0.25;
+}
+
+bool fused_supported(const LatticeDesc& L, const StepCoef& c) {
+    return fused_shape_ok(L, c) && L.periodic_x == L.periodic_y;
 }
 
 int fused_default_seg_rows(const LatticeDesc& L, int S) {

@@ -153,7 +153,7 @@ template <typename T>
 int sweep(const LatticeDesc& L, T* re, T* im, int axis, int parity, double a, double b,
           cudaStream_t st, int64_t* launches) {
     const int64_t n = axis == 0 ? L.nx : L.ny;
-    const int wrap = (L.periodic && parity == 1) ? 1 : 0;
+    const int wrap = ((axis == 0 ? L.periodic_x : L.periodic_y) && parity == 1) ? 1 : 0;
     int64_t pairs = parity == 0 ? n / 2 : (n - 1) / 2;
     if (wrap) pairs += 1;   // n even when periodic: (n-1)/2 inner pairs + the wrap pair = n/2
     if (pairs <= 0) return TS_OK;

@@ -25,7 +25,7 @@ struct StepCoef {
 struct LatticeDesc {
     int64_t nx, ny;
     int dtype;      // TS_F32 / TS_F64
-    int periodic;   // 0 closed, 1 periodic
+    int periodic_x, periodic_y;   // per axis: 0 closed, 1 periodic
 };
 
 // ---- generic per-sweep path (ts_generic.cu): in place, any nx, ny ------------------------------
@@ -39,7 +39,8 @@ int norm2_device(const LatticeDesc& L, const void* re, const void* im, double* d
 size_t norm_workspace_doubles();
 
 // ---- fused streaming path (ts_fused.cu): out of place, S steps per pass ------------------------
-bool fused_supported(const LatticeDesc& L, const StepCoef& c);
+bool fused_shape_ok(const LatticeDesc& L, const StepCoef& c);   // alignment and angle range only
+bool fused_supported(const LatticeDesc& L, const StepCoef& c);  // + same boundary on both axes
 // One pass: dst <- U2^S src.  S in 1..TS_MAX_FUSE.  seg_rows even, > 0.
 int fused_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
                void* dst_im, const StepCoef& c, const void* pot, int S, int seg_rows,

@@ -125,7 +125,7 @@ struct StreamCtx {
 // is accounted for in out_scale.
 // pot_yj / pot_yjm1: shared addresses of the potential rows yj (row 0 of its slot) and yj-1
 // (row 1 of the previous slot).
-template <typename T, bool PER, bool XEDGE, int S, int J>
+template <typename T, int BND, bool XEDGE, int S, int J>
 __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const StreamCtx<T>& c,
                                              int yj, Row4<T>& a0, Row4<T>& a1, Row4<T>& g,
                                              Row4<T>& h, uint32_t pot_yj, uint32_t pot_yjm1) {
@@ -174,7 +174,7 @@ __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const Str
 // 4S+2 sweeps instead of 7S.  Only the rounding differs from the literal sequence.
 //   in : (a0, a1) = rows (yj, yj+1) entering step; (g, h) = rows (yj-2, yj-1), h waiting for Yo
 //   out: (g, h) finished with this step; (a0, a1) held for the next iteration
-template <typename T, bool PER, bool XEDGE, int S, int J>
+template <typename T, int BND, bool XEDGE, int S, int J>
 __device__ __forceinline__ void stream_stage_nopot(const StreamParams<T>& p,
                                                    const StreamCtx<T>& c, int yj, Row4<T>& a0,
                                                    Row4<T>& a1, Row4<T>& g, Row4<T>& h) {
@@ -193,7 +193,7 @@ __device__ __forceinline__ void stream_stage_nopot(const StreamParams<T>& p,
 }
 
 // stages 0..S-1 of one iteration: the pair (x0, x1) flows through them, see the kernel
-template <typename T, bool POT, bool PER, bool XEDGE, int S, int J>
+template <typename T, bool POT, int BND, bool XEDGE, int S, int J>
 struct Stages {
     static __device__ __forceinline__ void run(const StreamParams<T>& p, const StreamCtx<T>& c,
                                                int y, int cs, int nst, uint32_t slotb,
@@ -210,20 +210,23 @@ struct Stages {
             int s1 = s0 - 1;      if (s1 < 0) s1 += nst;
             const uint32_t pot_yj = c.ring + s0 * slotb + 4 * ROWB;
             const uint32_t pot_yjm1 = c.ring + s1 * slotb + 6 * ROWB;
-            stream_stage<T, PER, XEDGE, S, J>(p, c, y - 2 * J, a0, a1, g, h, pot_yj, pot_yjm1);
+            stream_stage<T, BND, XEDGE, S, J>(p, c, y - 2 * J, a0, a1, g, h, pot_yj, pot_yjm1);
         } else {
-            stream_stage_nopot<T, PER, XEDGE, S, J>(p, c, y - 2 * J, a0, a1, g, h);
+            stream_stage_nopot<T, BND, XEDGE, S, J>(p, c, y - 2 * J, a0, a1, g, h);
         }
         x0 = g; x1 = h;   // (g, h) left the sub-step and flows on; (a0, a1) now waits in stage J
         if constexpr (J + 1 < S)
-            Stages<T, POT, PER, XEDGE, S, J + 1>::run(p, c, y, cs, nst, slotb, W, u, x0, x1);
+            Stages<T, POT, BND, XEDGE, S, J + 1>::run(p, c, y, cs, nst, slotb, W, u, x0, x1);
     }
 };
 
-template <typename T, int S, bool POT, bool PER, int MINB>
+template <typename T, int S, bool POT, int BND, int MINB>
 __global__ void __launch_bounds__(kWarps * 32, MINB)
 stream_kernel(const StreamParams<T> p) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
+    // BND: 0 = closed on both axes, 1 = periodic on both, 2 = periodic in x and closed in y (a row
+    // slab of a larger lattice, paper_1208_2407_b200/slab.py)
+    constexpr bool PERX = BND != 0, PERY = BND == 1;
     constexpr int R = POT ? S + 1 : 1;        // iterations a ring slot stays live after its arrival
     constexpr uint32_t ROWB = kStripSites * sizeof(T);
     constexpr int NROW = POT ? 8 : 4;         // re0 im0 re1 im1 [pr0 pi0 pr1 pi1]
@@ -240,10 +243,10 @@ stream_kernel(const StreamParams<T> p) {
     const int xs = x0 - p.halo;               // first column of the strip window
     const int xb = xs + 4 * lane;
     StreamCtx<T> c;
-    c.xvalid = PER ? true : (xb >= 0 && xb < p.nx);
-    c.xedge = !PER && (xs < 0 || xs + kStripSites > p.nx);
-    c.e.up = !PER && (xb == 0 || xb == p.nx);
-    c.e.dn = !PER && (xb + 4 == p.nx || xb + 4 == 0);
+    c.xvalid = PERX ? true : (xb >= 0 && xb < p.nx);
+    c.xedge = !PERX && (xs < 0 || xs + kStripSites > p.nx);
+    c.e.up = !PERX && (xb == 0 || xb == p.nx);
+    c.e.dn = !PERX && (xb + 4 == p.nx || xb + 4 == 0);
     c.ring = smem_u32(smem_raw) + warp * NST * SLOTB;
     c.lane_off = lane * 4 * sizeof(T);
     const uint32_t bars = smem_u32(smem_raw) + kWarps * NST * SLOTB + warp * NST * 8;
@@ -252,7 +255,7 @@ stream_kernel(const StreamParams<T> p) {
     // the strip window [xs, xs+128) as at most two contiguous global pieces (warp-uniform);
     // piece B (periodic wrap) always starts at global column 0
     int gx_a, off_a, len_a, len_b;
-    if (PER) {
+    if (PERX) {
         gx_a = wrap_index(xs, p.nx);
         off_a = 0;
         len_a = min(kStripSites, p.nx - gx_a);
@@ -282,13 +285,13 @@ stream_kernel(const StreamParams<T> p) {
     __syncwarp();
 
     // running row of the next fetch (warp-uniform): rows (fy, fy+1), element offset foff
-    int fy = PER ? wrap_index(y_in0, p.ny) : y_in0;
+    int fy = PERY ? wrap_index(y_in0, p.ny) : y_in0;
     int64_t foff = (int64_t)fy * p.nx;
     const int64_t plane_elems = (int64_t)p.nx * p.ny;
 
     // fetch the next row pair into ring slot `slot` (one elected lane issues all copies)
     auto issue = [&](int slot) {
-        const bool rowok = PER ? true : (fy >= 0 && fy < p.ny);
+        const bool rowok = PERY ? true : (fy >= 0 && fy < p.ny);
         if (leader) {
             const uint32_t bar = bars + 8 * slot;
             if (rowok) {
@@ -308,7 +311,7 @@ stream_kernel(const StreamParams<T> p) {
         }
         fy += 2;
         foff += 2 * (int64_t)p.nx;
-        if (PER && fy >= p.ny) { fy -= p.ny; foff -= plane_elems; }
+        if (PERY && fy >= p.ny) { fy -= p.ny; foff -= plane_elems; }
     };
 
     for (int k = 0; k < DIST; ++k)
@@ -360,7 +363,7 @@ stream_kernel(const StreamParams<T> p) {
                     zero_row(x0);
                     zero_row(x1);
                 }
-                Stages<T, POT, PER, XEDGE, S, 0>::run(p, c, y, cs, NST, SLOTB, W, U, x0, x1);
+                Stages<T, POT, BND, XEDGE, S, 0>::run(p, c, y, cs, NST, SLOTB, W, U, x0, x1);
                 if (it >= 2 * S && store_ok && y - 2 * S < y_out1) {
                     const int64_t off = (int64_t)(y - 2 * S) * p.nx + xb;
                     st4(p.dst_re + off, x0.re, p.out_scale);
@@ -376,12 +379,12 @@ stream_kernel(const StreamParams<T> p) {
         half(std::integral_constant<int, 1>{});
     }
     };   // run
-    const bool edge = !PER && (c.xedge || y_in0 < 0 || y_in0 + 2 * n_iter >= p.ny);
+    const bool edge = c.xedge || (!PERY && (y_in0 < 0 || y_in0 + 2 * n_iter >= p.ny));
     if (edge) run(std::true_type{});
     else run(std::false_type{});
 }
 
-template <typename T, int S, bool POT, bool PER>
+template <typename T, int S, bool POT, int BND>
 int launch(const StreamParams<T>& p, cudaStream_t st) {
     constexpr uint32_t SLOTB = (POT ? 8 : 4) * kStripSites * sizeof(T);
     const size_t smem = (size_t)kWarps * p.nst * (SLOTB + 8);
@@ -391,7 +394,7 @@ int launch(const StreamParams<T>& p, cudaStream_t st) {
 #define TS_MINB_F32 (S <= 4 ? 4 : 3)
 #endif
     constexpr int MINB = sizeof(T) == 4 ? TS_MINB_F32 : (S <= 2 ? 3 : 2);
-    auto kern = stream_kernel<T, S, POT, PER, MINB>;
+    auto kern = stream_kernel<T, S, POT, BND, MINB>;
     static size_t configured = 0;    // per instantiation
     if (smem > configured) {
         TS_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -405,10 +408,16 @@ int launch(const StreamParams<T>& p, cudaStream_t st) {
     return TS_OK;
 }
 
+template <typename T, int S, bool POT>
+int launch_b(const StreamParams<T>& p, int bnd, cudaStream_t st) {
+    if (bnd == 1) return launch<T, S, POT, 1>(p, st);
+    if (bnd == 2) return launch<T, S, POT, 2>(p, st);
+    return launch<T, S, POT, 0>(p, st);
+}
+
 template <typename T, int S>
-int launch_s(const StreamParams<T>& p, bool pot, bool per, cudaStream_t st) {
-    if (pot) return per ? launch<T, S, true, true>(p, st) : launch<T, S, true, false>(p, st);
-    return per ? launch<T, S, false, true>(p, st) : launch<T, S, false, false>(p, st);
+int launch_s(const StreamParams<T>& p, bool pot, int bnd, cudaStream_t st) {
+    return pot ? launch_b<T, S, true>(p, bnd, st) : launch_b<T, S, false>(p, bnd, st);
 }
 
 template <typename T>
@@ -465,7 +474,7 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
     }
     for (int j = S; j < TS_MAX_FUSE; ++j) { p.to[j] = T(0); p.sec_o[j] = T(1); p.te[j + 1] = T(0); }
     p.out_scale = (T)scale;
-    const bool per = L.periodic != 0;
+    const int per = L.periodic_x ? (L.periodic_y ? 1 : 2) : 0;
     switch (S) {
         case 1: return launch_s<T, 1>(p, pot != nullptr, per, st);
         case 2: return launch_s<T, 2>(p, pot != nullptr, per, st);
@@ -475,8 +484,8 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
     // deeper temporal blocking only where the ALU budget allows it: fp32 without a potential
     if constexpr (sizeof(T) == 4) {
         if (!pot) {
-            if (S == 5) return per ? launch<T, 5, false, true>(p, st) : launch<T, 5, false, false>(p, st);
-            if (S == 6) return per ? launch<T, 6, false, true>(p, st) : launch<T, 6, false, false>(p, st);
+            if (S == 5) return launch_b<T, 5, false>(p, per, st);
+            if (S == 6) return launch_b<T, 6, false>(p, per, st);
         }
     }
     set_error("stream_pass: steps per pass out of range");
@@ -487,7 +496,8 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
 
 bool stream_supported(const LatticeDesc& L, const StepCoef& c) {
     // the strip window must split into at most two contiguous pieces of a row
-    return fused_supported(L, c) && L.nx >= kStripSites;
+    // (closed in x with periodic in y is not instantiated)
+    return fused_shape_ok(L, c) && L.nx >= kStripSites && (L.periodic_x || !L.periodic_y);
 }
 
 int stream_max_steps(const LatticeDesc& L, bool pot) {

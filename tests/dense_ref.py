@@ -65,6 +65,21 @@ def step_unitary(nx, ny, periodic, theta, V=None, dt=1.0) -> np.ndarray:
     return Xe @ Xo @ Ye @ mid @ Ye @ Xo @ Xe
 
 
+def step_unitary_xy(nx, ny, periodic_x, periodic_y, theta, V=None, dt=1.0) -> np.ndarray:
+    """step_unitary with one boundary type per axis (a row slab: periodic in x, closed in y)."""
+    h = theta / 2.0
+    Xe = part_unitary(nx, ny, 0, 0, periodic_x, h)
+    Xo = part_unitary(nx, ny, 0, 1, periodic_x, h)
+    Ye = part_unitary(nx, ny, 1, 0, periodic_y, h)
+    if V is None:
+        mid = part_unitary(nx, ny, 1, 1, periodic_y, theta)
+    else:
+        Yo = part_unitary(nx, ny, 1, 1, periodic_y, h)
+        P = np.diag(np.exp(-1j * np.asarray(V, dtype=float).reshape(-1) * dt))
+        mid = Yo @ P @ Yo
+    return Xe @ Xo @ Ye @ mid @ Ye @ Xo @ Xe
+
+
 def exact_unitary(nx, ny, periodic, J, T, V=None) -> np.ndarray:
     """exp(-i H T), H = -J * Adj + diag(V): the thing the splitting approximates (Eq. 2)."""
     H = -J * full_adjacency(nx, ny, periodic)

@@ -1,0 +1,83 @@
+"""-m gpu: (1) the stream kernel with one boundary type per axis (ts_plan_create_xy) against
+oracle.evolve_xy; (2) the row-slab decomposition (slab.LocalGroup: all ranks stepped in turn on
+cuda:0, halos exchanged by copies) with the real kernels against the undivided oracle."""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+import pytest
+
+import gpu_util as G
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+TIGHT = {"f32": 2e-5, "f64": 5e-14}
+
+
+def coeffs(theta):
+    return (math.cos(theta / 2), math.sin(theta / 2), math.cos(theta), math.sin(theta))
+
+
+@pytest.mark.parametrize("nx,ny", [(128, 40), (380, 130)])
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("with_pot", [False, True])
+@pytest.mark.parametrize("fuse", [1, 3, 4, 6])
+@pytest.mark.parametrize("bx,by", [("periodic", "closed"), ("closed", "periodic")])
+def test_per_axis_boundaries(nx, ny, dtype, with_pot, fuse, bx, by):
+    import torch
+    from paper_1208_2407_b200.binding import Plan
+    if fuse > 4 and (with_pot or dtype == "f64"):
+        pytest.skip("S = 5, 6 exist only for fp32 without a potential")
+    dev = torch.device("cuda:0")
+    re, im, pot = G.random_inputs(nx, ny, dtype, 31 * nx + ny + fuse, with_pot)
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    plan = Plan(nx, ny, tdt, bx, by)
+    stream_path = bx == "periodic"       # (closed x, periodic y) runs on the per-sweep kernels
+    if stream_path:
+        plan.set_option("path", 2); plan.set_option("variant", 2)
+        plan.set_option("fuse_steps", fuse); plan.set_option("seg_rows", 16)
+    dre, dim = torch.from_numpy(re).to(dev), torch.from_numpy(im).to(dev)
+    dpot = None if pot is None else torch.from_numpy(pot).to(dev)
+    n = 9
+    plan.evolve(dre, dim, *coeffs(0.3), pot_phase=dpot, n_steps=n)
+    torch.cuda.synchronize()
+    assert plan.info("fused") == (1 if stream_path else 0)
+    wre, wim = re.astype(np.float64), im.astype(np.float64)
+    p64 = None if pot is None else (pot[0].astype(np.float64), pot[1].astype(np.float64))
+    oracle.evolve_xy(wre, wim, *coeffs(0.3), pot=p64, periodic_x=bx == "periodic",
+                     periodic_y=by == "periodic", n_steps=n)
+    err = max(np.abs(dre.cpu().numpy() - wre).max(), np.abs(dim.cpu().numpy() - wim).max())
+    assert err <= TIGHT[dtype] * 2, err
+    plan.destroy()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+@pytest.mark.parametrize("boundary", ["closed", "periodic"])
+@pytest.mark.parametrize("with_pot", [False, True])
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_slab_decomposition_matches_undivided_oracle(world, boundary, with_pot, dtype):
+    import torch
+    from paper_1208_2407_b200 import slab
+    dev = torch.device("cuda:0")
+    nx, ny, k, n = 380, 132, 6, 20          # exchange every 6 steps (halo 12 rows), 4 periods
+    re, im, pot = G.random_inputs(nx, ny, dtype, 99 + world, with_pot)
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    g = slab.LocalGroup(nx, ny, tdt, boundary, world, k, device=dev)
+    g.scatter(torch.from_numpy(re).to(dev), torch.from_numpy(im).to(dev),
+              None if pot is None else torch.from_numpy(pot).to(dev))
+    n0 = g.norm()
+    g.evolve(coeffs(0.3), n)
+    out_re = torch.empty((ny, nx), dtype=tdt, device=dev); out_im = torch.empty_like(out_re)
+    g.gather(out_re, out_im)
+    torch.cuda.synchronize()
+    n1 = g.norm()
+    wre, wim = re.astype(np.float64), im.astype(np.float64)
+    p64 = None if pot is None else (pot[0].astype(np.float64), pot[1].astype(np.float64))
+    oracle.evolve(wre, wim, *coeffs(0.3), pot=p64, periodic=boundary == "periodic", n_steps=n)
+    err = max(np.abs(out_re.cpu().numpy() - wre).max(), np.abs(out_im.cpu().numpy() - wim).max())
+    assert err <= TIGHT[dtype] * 3, err
+    assert abs(n0 / oracle.norm2(re.astype(np.float64), im.astype(np.float64)) - 1) < 1e-6
+    assert abs(n1 / n0 - 1) < (1e-4 if dtype == "f32" else 1e-12)
+    g.destroy()

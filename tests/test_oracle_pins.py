@@ -290,3 +290,28 @@ def test_periodic_rejects_odd_sizes():
     re, im = rand_state(4, 5, 1)
     with pytest.raises(ValueError):
         oracle.evolve(re, im, *coeffs(0.1), periodic=True, n_steps=1)
+
+
+# --- per-axis boundaries (row slabs of a domain decomposition) -----------------
+@pytest.mark.parametrize("px,py", [(True, False), (False, True), (True, True), (False, False)])
+@pytest.mark.parametrize("with_pot", [False, True])
+def test_evolve_xy_equals_dense_product_per_axis(px, py, with_pot):
+    from dense_ref import step_unitary_xy
+    nx, ny, theta = 6, 4, 0.37
+    rng = np.random.default_rng(17)
+    V = rng.uniform(-2, 2, (ny, nx)) if with_pot else None
+    re, im = rand_state(ny, nx, 21)
+    U = step_unitary_xy(nx, ny, px, py, theta, V)
+    want = U @ (U @ to_vec(re, im))
+    pot = None if V is None else (np.cos(V), -np.sin(V))
+    oracle.evolve_xy(re, im, *coeffs(theta), pot=pot, periodic_x=px, periodic_y=py, n_steps=2)
+    wr, wi = from_vec(want, ny, nx)
+    assert np.abs(re - wr).max() < 1e-13 and np.abs(im - wi).max() < 1e-13
+
+
+def test_evolve_xy_with_equal_boundaries_is_evolve():
+    re, im = rand_state(10, 12, 5)
+    r2, i2 = re.copy(), im.copy()
+    oracle.evolve(re, im, *coeffs(0.2), periodic=True, n_steps=3)
+    oracle.evolve_xy(r2, i2, *coeffs(0.2), periodic_x=True, periodic_y=True, n_steps=3)
+    assert np.array_equal(re, r2) and np.array_equal(im, i2)
