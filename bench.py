@@ -299,6 +299,112 @@ def run_gpu(args):
     return 0
 
 
+def run_gpu_slab(args):
+    """ONE lattice cut into row slabs (paper_1208_2407_b200/slab.py): with N > 1 ranks the global
+    lattice is nx x (ny * N) (weak scaling: every rank owns a slab of the config's size) and halos
+    travel over NCCL; with --slabs R on one GPU the config's lattice is cut into R slabs stepped in
+    turn (measures the cost of the decomposition itself: halo recomputation + exchange copies)."""
+    import torch
+    from paper_1208_2407_b200 import inputs, slab
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    cfg = inputs.CONFIGS[args.config]
+    tdt = torch.float32 if cfg.dtype == "f32" else torch.float64
+    eb = 4 if cfg.dtype == "f32" else 8
+    re, im, _ = inputs.device_state(cfg, dev)
+    pot = inputs.device_pot(cfg, dev)
+    k = args.exchange_every or slab.default_steps_per_exchange(tdt, pot is not None)
+    c = cfg.coeffs()
+    if world > 1:
+        comm = slab.DistComm()
+        obj = slab.Slab(cfg.nx, cfg.ny * world, tdt, cfg.boundary, rank, world, k, device=dev)
+        obj.set_state(re, im)
+        if pot is not None:
+            obj.set_potential(pot, comm)
+        evolve = lambda: obj.evolve(c, cfg.n_steps, comm)
+        norm = lambda: obj.norm(comm)
+        plans = [obj.plan]
+        n_slabs, halo = world, obj.H
+    else:
+        obj = slab.LocalGroup(cfg.nx, cfg.ny, tdt, cfg.boundary, max(1, args.slabs), k, device=dev)
+        obj.scatter(re, im, pot)
+        evolve = lambda: obj.evolve(c, cfg.n_steps)
+        norm = obj.norm
+        plans = [s.plan for s in obj.slabs]
+        n_slabs, halo = len(obj.slabs), obj.slabs[0].H
+    del re, im, pot
+    torch.cuda.empty_cache()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    n0 = norm()
+    for _ in range(args.warmup):
+        evolve()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    stream = torch.cuda.current_stream()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0 = time.time()
+    e0.record(stream)
+    for _ in range(args.steps):
+        evolve()
+    e1.record(stream)
+    barrier()
+    t1 = time.time()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop(t0, t1) if rank == 0 else None
+    if dist is not None:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    n1 = norm()
+    S = max(1, plans[0].info("fuse_steps"))
+    periods = -(-cfg.n_steps // k)
+    launches = sum(p.info("launches") for p in plans) * periods      # last period may be shorter
+    sites = cfg.sites * world
+    value = sites * cfg.n_steps * args.steps / (ms * 1e-3)
+    if rank != 0:
+        return 0
+    peak, peak_src = load_peaks()
+    bytes_per_site_step = (4 * eb + (2 * eb if cfg.has_pot else 0)) / S
+    achieved = value / world * bytes_per_site_step / 1e9
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
+        "config": {"workload": workload_text(cfg) + (f", stacked {world}x in y" if world > 1 else ""),
+                   "parallelism": f"row slabs x{n_slabs}, halo {halo} rows exchanged every {k} steps"
+                                  + (" over NCCL" if world > 1 else " (one GPU, slabs stepped in turn)"),
+                   "fuse_steps": S, "norm2_before": n0, "norm_drift": n1 / n0 - 1,
+                   "l2": "state far larger than the 126 MB L2; no flush"},
+        "clocks": clocks, "gpu_launches": launches * args.steps,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": None,
+                     "kernel": f"stream_kernel<{cfg.dtype}, S={S}> on slabs (per GPU, whole call "
+                               "incl. halo exchange)", "peak_source": peak_src},
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -308,6 +414,12 @@ def main():
     ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--fuse-steps", type=int, default=0)
     ap.add_argument("--seg-rows", type=int, default=0)
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent lattices per GPU (default, north_star) or one lattice "
+                         "cut into row slabs with NCCL halo exchange")
+    ap.add_argument("--slabs", type=int, default=0,
+                    help="N = 1: cut the lattice into this many slabs on the one GPU")
+    ap.add_argument("--exchange-every", type=int, default=0, help="steps between halo exchanges")
     ap.add_argument("--cpu-budget", type=float, default=1.5e9,
                     help="site-steps of oracle work in the cpu_baseline leg")
     args = ap.parse_args()
@@ -315,6 +427,8 @@ def main():
         args.warmup = 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.decomp == "slab" or args.slabs > 1:
+        return run_gpu_slab(args)
     return run_gpu(args)
 
 

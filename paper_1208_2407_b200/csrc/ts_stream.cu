@@ -119,10 +119,11 @@ struct StreamCtx {
 // One second-order sub-step (stage J of S) of the register pipeline, WITH a potential.
 //   in : (a0, a1) = rows (yj, yj+1) before the step; (g, h) = rows (yj-2, yj-1) in mid-step state
 //   out: (g, h) = rows (yj-2, yj-1) after the step; (a0, a1) = rows (yj, yj+1) in mid-step state
-// Between two chained sub-steps the closing X-even half sweep of one and the opening X-even
-// half sweep of the next act on the same rows back to back and are applied as ONE sweep by the
-// sum of the two half angles (te[J]) at the start of the later sub-step; the deferred cosine
-// is accounted for in out_scale.
+// Between two chained sub-steps the closing Y-even, X-odd, X-even half sweeps of one and the
+// opening X-even, X-odd, Y-even half sweeps of the next act on the same rows; X sweeps commute
+// with Y sweeps, so the two X-even and the two Y-even half sweeps are each applied as ONE sweep
+// by the sum of the two half angles (te[J]) in the later sub-step: 6 sweeps + P per sub-step
+// instead of 8 + P.  The deferred cosines are accounted for in out_scale.
 // pot_yj / pot_yjm1: shared addresses of the potential rows yj (row 0 of its slot) and yj-1
 // (row 1 of the previous slot).
 template <typename T, int BND, bool XEDGE, int S, int J>
@@ -130,10 +131,13 @@ __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const Str
                                              int yj, Row4<T>& a0, Row4<T>& a1, Row4<T>& g,
                                              Row4<T>& h, uint32_t pot_yj, uint32_t pot_yjm1) {
     constexpr uint32_t ROWB = kStripSites * sizeof(T);
+    constexpr bool LAST = J == S - 1;
     const T th = p.to[J];
     xe(a0, p.te[J]); xe(a1, p.te[J]);
     xo<T, XEDGE>(a0, th, p.sec_o[J], c.e); xo<T, XEDGE>(a1, th, p.sec_o[J], c.e);
-    ypair(a0, a1, th);
+    // opening Y-even sweep, merged with the closing one of the previous sub-step (only X sweeps
+    // lie between the two, and those commute with it)
+    ypair(a0, a1, p.te[J]);
     // closed lattice: the vertical-odd pair (yj-1, yj) does not exist at yj = 0 and yj = ny; the
     // ghost row is zero and stays zero (coupling 0), the real row takes 1/a per omitted sweep
     const bool yedge = XEDGE && (yj == 0 || yj == p.ny);
@@ -160,9 +164,9 @@ __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const Str
         const T sy = yedge ? p.sec_o[J] * p.sec_o[J] : T(1);
         scale_row(h, sy); scale_row(a0, sy);
     }
-    ypair(g, h, th);
+    if (LAST) ypair(g, h, p.te[S]);
     xo<T, XEDGE>(g, th, p.sec_o[J], c.e); xo<T, XEDGE>(h, th, p.sec_o[J], c.e);
-    if (J == S - 1) { xe(g, p.te[S]); xe(h, p.te[S]); }
+    if (LAST) { xe(g, p.te[S]); xe(h, p.te[S]); }
 }
 
 // The same sub-step WITHOUT a potential, regrouped.  Horizontal sweeps act inside a row and
@@ -448,7 +452,7 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
         p.te[0] = (T)(f.b_h / f.a_h);
         p.te[S] = (T)(l.b_h / l.a_h);
         const double ends = f.a_h * l.a_h;
-        scale *= pot ? ends : ends * ends;           // X only, or X and Y (regrouped)
+        scale *= ends * ends;                        // X-even and Y-even
     }
     for (int j = 1; j < S; ++j) {
         const StepCoef& u = subs[j - 1];
@@ -456,15 +460,15 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
         const double cm = u.a_h * v.a_h - u.b_h * v.b_h;
         const double sm = u.a_h * v.b_h + u.b_h * v.a_h;
         p.te[j] = (T)(sm / cm);
-        scale *= pot ? cm : cm * cm;
+        scale *= cm * cm;
     }
     for (int j = 0; j < S; ++j) {
         const StepCoef& v = subs[j];
         if (pot) {
-            // Xo, Ye, Yo at the half angle, each twice per sub-step
+            // Xo, Yo at the half angle, each twice per sub-step
             p.to[j] = (T)(v.b_h / v.a_h);
             p.sec_o[j] = (T)(1.0 / v.a_h);
-            scale *= pow(v.a_h, 6);
+            scale *= pow(v.a_h, 4);
         } else {
             // Xo and Yo at the full angle, once each
             p.to[j] = (T)(v.b_f / v.a_f);

@@ -51,6 +51,15 @@ def neighbours(rank: int, world: int, periodic_y: bool) -> Neighbours:
     return Neighbours(rank - 1 if rank > 0 else None, rank + 1 if rank < world - 1 else None)
 
 
+def default_steps_per_exchange(dtype, with_pot: bool) -> int:
+    """Two fused passes of the stream kernel's default depth (csrc/ts_fused.cu::
+    fused_default_steps), so that every local ts_evolve ends in the caller's planes."""
+    import torch
+    if dtype == torch.float32:
+        return 6 if with_pot else 12
+    return 6 if with_pot else 8
+
+
 class DistComm:
     """Halo exchange over torch.distributed (NCCL for CUDA tensors, gloo for CPU tensors)."""
 
