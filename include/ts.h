@@ -102,6 +102,23 @@ int ts_evolve_u4(ts_plan* plan, void* psi_re, void* psi_im, double theta,
                  int64_t n_steps, void* cuda_stream);
 
 /*
+ * ts_evolve_sep -- ts_evolve for a SEPARABLE potential V(x, y) = Vx(x) + Vy(y) (the harmonic trap
+ * of the benchmark configs is one): the phase of the diagonal step factorises,
+ * exp(-i V dt) = px(x) * py(y), and is passed as two vectors instead of two planes
+ * (the remark that a general potential "always adds a cost": this one adds
+ * arithmetic but no memory traffic).
+ *   phase_x   DEVICE pointer, 2*nx elements of the plan's dtype: Re px[0..nx), then Im px[0..nx).
+ *   phase_y   DEVICE pointer, 2*ny elements: Re py, then Im py.   Both 16-byte aligned.
+ * The step is the 9-stage step of ts_evolve with P(x, y) = px(x) py(y) (complex product, formed
+ * in the plan's dtype).  The TMA ring kernel keeps px in registers and reads py through L1, so a
+ * pass moves 16 B (fp32) per site like the potential-free step; other paths first write the
+ * product out as planes into plan-owned scratch.  Other arguments and errors as for ts_evolve.
+ */
+int ts_evolve_sep(ts_plan* plan, void* psi_re, void* psi_im,
+                  double a_half, double b_half, double a_full, double b_full,
+                  const void* phase_x, const void* phase_y, int64_t n_steps, void* cuda_stream);
+
+/*
  * ts_norm -- squared norm sum |psi|^2, accumulated in double for either dtype.
  *   psi_re, psi_im   DEVICE pointers as above (read only).
  *   out_norm2_host   HOST pointer to one double, written before the call returns.

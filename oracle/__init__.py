@@ -138,6 +138,20 @@ def evolve_xy(re, im, a_half, b_half, a_full, b_full, pot=None, periodic_x=False
         sweep(re, im, 0, 0, a_half, b_half, periodic_x)
 
 
+def evolve_sep(re, im, a_half, b_half, a_full, b_full, phase_x, phase_y, periodic=False,
+               n_steps=1) -> None:
+    """In place: the 9-stage step with a SEPARABLE potential phase P(x, y) = px(x) * py(y),
+    phase_x = (Re px, Im px) over x, phase_y likewise over y (float64).  By definition the
+    diagonal step multiplies site (x, y) by that complex product, so this is ``evolve`` with the
+    product written out as planes (exp(-i dt H0) with V = Vx + Vy)."""
+    px = np.asarray(phase_x[0], dtype=np.float64) + 1j * np.asarray(phase_x[1], dtype=np.float64)
+    py = np.asarray(phase_y[0], dtype=np.float64) + 1j * np.asarray(phase_y[1], dtype=np.float64)
+    P = py[:, None] * px[None, :]
+    evolve(re, im, a_half, b_half, a_full, b_full,
+           pot=(np.ascontiguousarray(P.real), np.ascontiguousarray(P.imag)), periodic=periodic,
+           n_steps=n_steps)
+
+
 # p of Eq. 4 (PAPER.md:95-101): p = (4 - 4^(1/3))^-1
 U4_P = 1.0 / (4.0 - 4.0 ** (1.0 / 3.0))
 

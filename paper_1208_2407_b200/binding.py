@@ -13,7 +13,8 @@ TS_MAX_FUSE = 6
 _LIB_PATH = Path(__file__).resolve().parent / "libts.so"
 _lib = None
 
-SYMBOLS = ["ts_plan_create", "ts_plan_create_xy", "ts_evolve", "ts_evolve_u4", "ts_norm", "ts_evolve_host", "ts_plan_set_option",
+SYMBOLS = ["ts_plan_create", "ts_plan_create_xy", "ts_evolve", "ts_evolve_u4", "ts_evolve_sep",
+           "ts_norm", "ts_evolve_host", "ts_plan_set_option",
            "ts_plan_get_info", "ts_plan_destroy", "ts_last_error"]
 
 
@@ -40,6 +41,8 @@ def lib():
         L.ts_evolve.restype = i32
         L.ts_evolve_u4.argtypes = [vp, vp, vp, dbl, vp, vp, i64, vp]
         L.ts_evolve_u4.restype = i32
+        L.ts_evolve_sep.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp, vp, i64, vp]
+        L.ts_evolve_sep.restype = i32
         L.ts_norm.argtypes = [vp, vp, vp, ctypes.POINTER(dbl), vp]
         L.ts_norm.restype = i32
         L.ts_evolve_host.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp, i64]
@@ -148,6 +151,20 @@ class Plan:
                                   ctypes.c_void_p(psi_im.data_ptr()), float(theta),
                                   self._pot_ptr(pot_phase_p), self._pot_ptr(pot_phase_q),
                                   int(n_steps), _stream_handle(stream)))
+
+    def evolve_sep(self, psi_re, psi_im, a_half, b_half, a_full, b_full, phase_x, phase_y,
+                   n_steps=1, stream=None):
+        """ts_evolve_sep: separable potential phase, phase_x [2][nx], phase_y [2][ny] (CUDA)."""
+        self._planes(psi_re, psi_im)
+        for t, n in ((phase_x, self.nx), (phase_y, self.ny)):
+            if t.dtype != self.dtype or tuple(t.shape) != (2, n) or not t.is_contiguous() \
+                    or not t.is_cuda:
+                raise ValueError("phase_x / phase_y must be contiguous CUDA tensors [2][n]")
+        _check(lib().ts_evolve_sep(self._h, ctypes.c_void_p(psi_re.data_ptr()),
+                                   ctypes.c_void_p(psi_im.data_ptr()), a_half, b_half, a_full,
+                                   b_full, ctypes.c_void_p(phase_x.data_ptr()),
+                                   ctypes.c_void_p(phase_y.data_ptr()), int(n_steps),
+                                   _stream_handle(stream)))
 
     def evolve_host(self, psi_re, psi_im, a_half, b_half, a_full, b_full, pot_phase=None,
                     n_steps=1):

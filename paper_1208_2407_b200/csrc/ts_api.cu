@@ -33,6 +33,7 @@ struct ts_plan {
     void* host_re;
     void* host_im;
     void* host_pot;
+    void* sep_pot;            // separable phase written out as planes (paths without mode 2)
     cudaStream_t own_stream;
     // options
     int64_t opt_path, opt_fuse, opt_seg, opt_variant, opt_slots;
@@ -126,6 +127,7 @@ int ts_plan_destroy(ts_plan* plan) {
     cudaFree(plan->host_re);
     cudaFree(plan->host_im);
     cudaFree(plan->host_pot);
+    cudaFree(plan->sep_pot);
     if (plan->own_stream) cudaStreamDestroy(plan->own_stream);
     delete plan;
     return TS_OK;
@@ -172,8 +174,12 @@ namespace {
 
 struct SubStep {
     ts::StepCoef c;
-    const void* pot;   // device phase planes of this sub-step or nullptr
+    ts::Phase ph;      // the diagonal step of this sub-step
 };
+
+bool same_phase(const ts::Phase& a, const ts::Phase& b) {
+    return a.mode == b.mode && a.planes == b.planes && a.px == b.px && a.py == b.py;
+}
 
 // psi <- (U2(pat[P-1]) ... U2(pat[0]))^n_repeat psi: the engine behind ts_evolve (P = 1) and
 // ts_evolve_u4 (P = 5).  Consecutive sub-steps that share a potential-phase array are fused into
@@ -188,19 +194,25 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
     if (!aligned16(psi_re) || !aligned16(psi_im))
         return fail(TS_EINVAL, "device pointers must be 16-byte aligned");
     if (overlap(psi_re, psi_im, plane_bytes)) return fail(TS_EINVAL, "psi_re and psi_im overlap");
-    bool any_pot = false, can_v1 = true, can_stream = true;
+    bool any_pot = false, any_sep = false, can_v1 = true, can_stream = true;
     for (int k = 0; k < period; ++k) {
         const ts::StepCoef& c = pat[k].c;
         if (!coef_ok(c.a_h, c.b_h) || !coef_ok(c.a_f, c.b_f))
             return fail(TS_EINVAL, "coefficients must be finite with |a^2 + b^2 - 1| <= 1e-6");
-        const void* pot = pat[k].pot;
-        if (pot) {
+        const ts::Phase& ph = pat[k].ph;
+        if (ph.mode == 1) {
+            const void* pot = ph.planes;
             any_pot = true;
             if (!aligned16(pot)) return fail(TS_EINVAL, "device pointers must be 16-byte aligned");
             if (overlap(pot, psi_re, plane_bytes) || overlap(pot, psi_im, plane_bytes) ||
                 overlap((const char*)pot + plane_bytes, psi_re, plane_bytes) ||
                 overlap((const char*)pot + plane_bytes, psi_im, plane_bytes))
                 return fail(TS_EINVAL, "pot_phase overlaps psi");
+        } else if (ph.mode == 2) {
+            any_pot = any_sep = true;
+            if (!ph.px || !ph.py) return fail(TS_EINVAL, "NULL separable phase vector");
+            if (!aligned16(ph.px) || !aligned16(ph.py))
+                return fail(TS_EINVAL, "device pointers must be 16-byte aligned");
         }
         can_v1 = can_v1 && ts::fused_supported(L, c);
         can_stream = can_stream && ts::stream_supported(L, c);
@@ -219,14 +231,34 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
     if (plan->opt_path == 2 && !can_fuse)
         return fail(TS_EUNSUPPORTED,
                     "fused kernel needs nx % 4 == 0, even ny and cos(theta) > 0.25");
+    const bool use_stream_early = can_stream && plan->opt_variant != 1 && plan->opt_path != 1 &&
+                                  can_fuse;
+    // separable factors are consumed directly only by the TMA ring kernel; every other path gets
+    // them written out as planes (one array: period-1 patterns only)
+    SubStep expanded;
+    if (any_sep && !use_stream_early) {
+        if (period != 1) return fail(TS_EUNSUPPORTED, "separable phases of a multi-sub-step pattern need the TMA ring kernel");
+        rc = ensure_alloc(&plan->sep_pot, 2 * plane_bytes);
+        if (rc != TS_OK) return rc;
+        rc = ts::expand_separable(L, pat[0].ph.px, pat[0].ph.py, plan->sep_pot, st);
+        if (rc != TS_OK) return rc;
+        ++plan->info_launches;
+        expanded = pat[0];
+        expanded.ph = ts::Phase{1, plan->sep_pot, nullptr, nullptr};
+        pat = &expanded;
+    }
     if (plan->opt_path == 1 || !can_fuse) {
-        if (period == 1)
-            return ts::generic_evolve(L, psi_re, psi_im, pat[0].c, pat[0].pot, n_repeat, st,
-                                      &plan->info_launches);
+        const int64_t l0 = plan->info_launches;
+        if (period == 1) {
+            rc = ts::generic_evolve(L, psi_re, psi_im, pat[0].c, pat[0].ph.planes, n_repeat, st,
+                                    &plan->info_launches);
+            plan->info_launches += l0;
+            return rc;
+        }
         for (int64_t i = 0; i < n_sub; ++i) {
             const SubStep& s = pat[i % period];
             int64_t launches = 0;
-            rc = ts::generic_evolve(L, psi_re, psi_im, s.c, s.pot, 1, st, &launches);
+            rc = ts::generic_evolve(L, psi_re, psi_im, s.c, s.ph.planes, 1, st, &launches);
             if (rc != TS_OK) return rc;
             plan->info_launches += launches;
         }
@@ -242,7 +274,9 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
     if (plan->opt_variant == 1 && !can_v1)
         return fail(TS_EUNSUPPORTED, "the register-prefetch kernel needs one boundary type on both axes");
     const bool use_stream = can_stream && plan->opt_variant != 1;
-    int S = plan->opt_fuse ? (int)plan->opt_fuse : ts::fused_default_steps(L, any_pot);
+    int S = plan->opt_fuse ? (int)plan->opt_fuse
+                           : (any_sep && use_stream ? ts::stream_default_steps_sep(L)
+                                                    : ts::fused_default_steps(L, any_pot));
     const int s_max = use_stream ? ts::stream_max_steps(L, any_pot) : 4;
     if (S > s_max) {
         if (plan->opt_fuse)
@@ -258,19 +292,19 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
         // the run of sub-steps of this pass: same potential array; the register-prefetch kernel
         // (variant 1) also needs equal angles
         ts::StepCoef subs[TS_MAX_FUSE];
-        const void* pot = pat[i % period].pot;
+        const ts::Phase ph = pat[i % period].ph;
         int s = 0;
         while (s < S && i + s < n_sub) {
             const SubStep& x = pat[(i + s) % period];
-            if (x.pot != pot) break;
+            if (!same_phase(x.ph, ph)) break;
             if (!use_stream && s > 0 && memcmp(&x.c, &subs[0], sizeof(ts::StepCoef)) != 0) break;
             subs[s++] = x.c;
         }
         if (use_stream)
-            rc = ts::stream_pass(L, cur_re, cur_im, nxt_re, nxt_im, subs, pot, s, seg,
+            rc = ts::stream_pass(L, cur_re, cur_im, nxt_re, nxt_im, subs, ph, s, seg,
                                  (int)plan->opt_slots, st);
         else
-            rc = ts::fused_pass(L, cur_re, cur_im, nxt_re, nxt_im, subs[0], pot, s, seg, st);
+            rc = ts::fused_pass(L, cur_re, cur_im, nxt_re, nxt_im, subs[0], ph.planes, s, seg, st);
         if (rc != TS_OK) return rc;
         void* t;
         t = cur_re; cur_re = nxt_re; nxt_re = t;
@@ -296,7 +330,16 @@ extern "C" {
 
 int ts_evolve(ts_plan* plan, void* psi_re, void* psi_im, double a_half, double b_half,
               double a_full, double b_full, const void* pot, int64_t n_steps, void* cuda_stream) {
-    const SubStep one{{a_half, b_half, a_full, b_full}, pot};
+    const SubStep one{{a_half, b_half, a_full, b_full},
+                      ts::Phase{pot ? 1 : 0, pot, nullptr, nullptr}};
+    return evolve_pattern(plan, psi_re, psi_im, &one, 1, n_steps, cuda_stream);
+}
+
+int ts_evolve_sep(ts_plan* plan, void* psi_re, void* psi_im, double a_half, double b_half,
+                  double a_full, double b_full, const void* phase_x, const void* phase_y,
+                  int64_t n_steps, void* cuda_stream) {
+    if (!phase_x || !phase_y) return fail(TS_EINVAL, "NULL separable phase vector");
+    const SubStep one{{a_half, b_half, a_full, b_full}, ts::Phase{2, nullptr, phase_x, phase_y}};
     return evolve_pattern(plan, psi_re, psi_im, &one, 1, n_steps, cuda_stream);
 }
 
@@ -312,7 +355,8 @@ int ts_evolve_u4(ts_plan* plan, void* psi_re, void* psi_im, double theta, const 
     for (int k = 0; k < 5; ++k) {
         const double th = frac[k] * theta;
         pat[k].c = ts::StepCoef{cos(0.5 * th), sin(0.5 * th), cos(th), sin(th)};
-        pat[k].pot = k == 2 ? pot_q : pot_p;
+        const void* pot = k == 2 ? pot_q : pot_p;
+        pat[k].ph = ts::Phase{pot ? 1 : 0, pot, nullptr, nullptr};
     }
     return evolve_pattern(plan, psi_re, psi_im, pat, 5, n_steps, cuda_stream);
 }

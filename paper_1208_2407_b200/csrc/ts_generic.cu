@@ -213,6 +213,34 @@ int generic_evolve(const LatticeDesc& L, void* re, void* im, const StepCoef& c, 
                             launches);
 }
 
+namespace {
+template <typename T>
+__global__ void expand_separable_kernel(const T* __restrict__ px, const T* __restrict__ py,
+                                        T* __restrict__ pot, int64_t nx, int64_t ny) {
+    const int64_t n = nx * ny;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t x = i % nx, y = i / nx;
+        const T xr = px[x], xi = px[nx + x], yr = py[y], yi = py[ny + y];
+        pot[i] = xr * yr - xi * yi;
+        pot[n + i] = xr * yi + xi * yr;
+    }
+}
+}  // namespace
+
+int expand_separable(const LatticeDesc& L, const void* px, const void* py, void* pot,
+                     cudaStream_t st) {
+    const int64_t n = L.nx * L.ny;
+    if (L.dtype == TS_F32)
+        expand_separable_kernel<float><<<grid_for(n, 256), 256, 0, st>>>(
+            (const float*)px, (const float*)py, (float*)pot, L.nx, L.ny);
+    else
+        expand_separable_kernel<double><<<grid_for(n, 256), 256, 0, st>>>(
+            (const double*)px, (const double*)py, (double*)pot, L.nx, L.ny);
+    TS_CUDA_TRY(cudaGetLastError());
+    return TS_OK;
+}
+
 size_t norm_workspace_doubles() { return kNormBlocks + 1; }
 
 int norm2_device(const LatticeDesc& L, const void* re, const void* im, double* d_work,

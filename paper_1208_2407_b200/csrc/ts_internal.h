@@ -22,6 +22,15 @@ struct StepCoef {
     double a_h, b_h, a_f, b_f;
 };
 
+// The diagonal step P of a sub-step: none, full phase planes [2][ny][nx], or separable factors
+// px [2][nx], py [2][ny] with P(x, y) = px(x) * py(y) (device pointers of the plan's dtype).
+struct Phase {
+    int mode;             // 0 none, 1 planes, 2 separable
+    const void* planes;
+    const void* px;
+    const void* py;
+};
+
 struct LatticeDesc {
     int64_t nx, ny;
     int dtype;      // TS_F32 / TS_F64
@@ -50,12 +59,16 @@ int fused_default_seg_rows(const LatticeDesc& L, int S);
 // ---- fused streaming path v2 (ts_stream.cu): TMA bulk copies into a per-warp smem ring ---------
 bool stream_supported(const LatticeDesc& L, const StepCoef& c);
 int stream_max_steps(const LatticeDesc& L, bool pot);   // 6 for fp32 without potential, else 4
+int stream_default_steps_sep(const LatticeDesc& L);     // sub-steps per pass, separable phase
 int stream_default_slots(const LatticeDesc& L, int S, bool pot);
 // One pass: dst <- U2(subs[S-1]) ... U2(subs[0]) src; the S sub-steps may have different angles
 // (fourth-order step, Eq. 4) but share one potential-phase array.
 int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
-                void* dst_im, const StepCoef* subs, const void* pot, int S, int seg_rows, int nst,
+                void* dst_im, const StepCoef* subs, const Phase& ph, int S, int seg_rows, int nst,
                 cudaStream_t st);
+// pot[2][ny][nx] <- px (x) py: the separable factors written out for paths that take planes
+int expand_separable(const LatticeDesc& L, const void* px, const void* py, void* pot,
+                     cudaStream_t st);
 int fused_default_steps(const LatticeDesc& L, bool pot);
 
 }  // namespace ts

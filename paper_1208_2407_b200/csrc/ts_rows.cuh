@@ -218,6 +218,35 @@ __device__ __forceinline__ void phase_row(Row4<float>& r, const float (&pr)[4],
 }
 #endif
 
+// separable potential: psi <- psi * (px + i px') * (py + i py') on one row; px per site of the
+// lane (registers), py one value for the row
+template <typename T>
+__device__ __forceinline__ void sep_phase_row(Row4<T>& r, const T (&pxr)[4], const T (&pxi)[4],
+                                              T pyr, T pyi) {
+    T wr[4], wi[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        wr[i] = fma(-pxi[i], pyi, pxr[i] * pyr);
+        wi[i] = fma(pxi[i], pyr, pxr[i] * pyi);
+    }
+    phase_row(r, wr, wi);
+}
+#ifndef TS_SCALAR_F32
+__device__ __forceinline__ void sep_phase_row(Row4<float>& r, const float (&pxr)[4],
+                                              const float (&pxi)[4], float pyr, float pyi) {
+    float wr[4], wi[4];
+#pragma unroll
+    for (int k = 0; k < 4; k += 2) {
+        float m0, m1, n0, n1;
+        mul2v(m0, m1, pxr[k], pxr[k + 1], pyr, pyr);
+        mul2v(n0, n1, pxr[k], pxr[k + 1], pyi, pyi);
+        fma2(wr[k], wr[k + 1], -pyi, pxi[k], pxi[k + 1], m0, m1);
+        fma2(wi[k], wi[k + 1], pyr, pxi[k], pxi[k + 1], n0, n1);
+    }
+    phase_row(r, wr, wi);
+}
+#endif
+
 __device__ __forceinline__ int wrap_index(int v, int n) {
     while (v < 0) v += n;
     while (v >= n) v -= n;

@@ -34,8 +34,12 @@ struct StreamParams {
     const T* src_im;
     T* dst_re;
     T* dst_im;
-    const T* pot_re;
+    const T* pot_re;      // phase planes [ny][nx] (phase mode 1)
     const T* pot_im;
+    const T* px_re;       // separable phase (mode 2): P(x, y) = px(x) * py(y), px [nx], py [ny]
+    const T* px_im;
+    const T* py_re;
+    const T* py_im;
     int nx, ny;
     int n_strips, wi, halo, seg_rows;
     int nst;        // ring slots per warp
@@ -112,6 +116,7 @@ struct StreamCtx {
     bool xvalid;         // lane's sites exist (always when periodic)
     bool xedge;          // warp-uniform: strip touches a closed edge in x
     XCut e;              // where the lane's cross-lane X-odd pairs meet a closed edge
+    T pxr[4], pxi[4];    // separable potential: phase factor of the lane's four columns
     uint32_t ring;       // shared address of the warp's slot ring
     uint32_t lane_off;   // byte offset of the lane's 4 sites inside a row chunk
 };
@@ -126,7 +131,7 @@ struct StreamCtx {
 // instead of 8 + P.  The deferred cosines are accounted for in out_scale.
 // pot_yj / pot_yjm1: shared addresses of the potential rows yj (row 0 of its slot) and yj-1
 // (row 1 of the previous slot).
-template <typename T, int BND, bool XEDGE, int S, int J>
+template <typename T, int PM, int BND, bool XEDGE, int S, int J>
 __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const StreamCtx<T>& c,
                                              int yj, Row4<T>& a0, Row4<T>& a1, Row4<T>& g,
                                              Row4<T>& h, uint32_t pot_yj, uint32_t pot_yjm1) {
@@ -146,17 +151,28 @@ __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const Str
     {
         const bool lo_ok = !XEDGE || (c.xvalid && yj - 1 >= 0 && yj - 1 < p.ny);
         const bool hi_ok = !XEDGE || (c.xvalid && yj >= 0 && yj < p.ny);
-        if (lo_ok) {
-            T pr[4], pi[4];
-            lds4(pot_yjm1 + c.lane_off, pr);
-            lds4(pot_yjm1 + ROWB + c.lane_off, pi);
-            phase_row(h, pr, pi);
-        }
-        if (hi_ok) {
-            T pr[4], pi[4];
-            lds4(pot_yj + c.lane_off, pr);
-            lds4(pot_yj + ROWB + c.lane_off, pi);
-            phase_row(a0, pr, pi);
+        if (PM == 2) {
+            // separable: the row factors come through L1 (one address per warp), the column
+            // factors sit in registers; ghost rows are zero, so any finite factor will do there
+            constexpr bool PERY = BND == 1;
+            int ylo = yj - 1, yhi = yj;
+            if (PERY) { ylo = wrap_index(ylo, p.ny); yhi = wrap_index(yhi, p.ny); }
+            else { ylo = min(max(ylo, 0), p.ny - 1); yhi = min(max(yhi, 0), p.ny - 1); }
+            sep_phase_row(h, c.pxr, c.pxi, __ldg(p.py_re + ylo), __ldg(p.py_im + ylo));
+            sep_phase_row(a0, c.pxr, c.pxi, __ldg(p.py_re + yhi), __ldg(p.py_im + yhi));
+        } else {
+            if (lo_ok) {
+                T pr[4], pi[4];
+                lds4(pot_yjm1 + c.lane_off, pr);
+                lds4(pot_yjm1 + ROWB + c.lane_off, pi);
+                phase_row(h, pr, pi);
+            }
+            if (hi_ok) {
+                T pr[4], pi[4];
+                lds4(pot_yj + c.lane_off, pr);
+                lds4(pot_yj + ROWB + c.lane_off, pi);
+                phase_row(a0, pr, pi);
+            }
         }
     }
     ypair(h, a0, t_yo);
@@ -197,7 +213,7 @@ __device__ __forceinline__ void stream_stage_nopot(const StreamParams<T>& p,
 }
 
 // stages 0..S-1 of one iteration: the pair (x0, x1) flows through them, see the kernel
-template <typename T, bool POT, int BND, bool XEDGE, int S, int J>
+template <typename T, int PM, int BND, bool XEDGE, int S, int J>
 struct Stages {
     static __device__ __forceinline__ void run(const StreamParams<T>& p, const StreamCtx<T>& c,
                                                int y, int cs, int nst, uint32_t slotb,
@@ -209,28 +225,31 @@ struct Stages {
         Row4<T>& g = W[J][u ^ 1][0];
         Row4<T>& h = W[J][u ^ 1][1];
         a0 = x0; a1 = x1;
-        if (POT) {
+        if (PM == 1) {
             int s0 = cs - J;      if (s0 < 0) s0 += nst;
             int s1 = s0 - 1;      if (s1 < 0) s1 += nst;
             const uint32_t pot_yj = c.ring + s0 * slotb + 4 * ROWB;
             const uint32_t pot_yjm1 = c.ring + s1 * slotb + 6 * ROWB;
-            stream_stage<T, BND, XEDGE, S, J>(p, c, y - 2 * J, a0, a1, g, h, pot_yj, pot_yjm1);
+            stream_stage<T, 1, BND, XEDGE, S, J>(p, c, y - 2 * J, a0, a1, g, h, pot_yj, pot_yjm1);
+        } else if (PM == 2) {
+            stream_stage<T, 2, BND, XEDGE, S, J>(p, c, y - 2 * J, a0, a1, g, h, 0, 0);
         } else {
             stream_stage_nopot<T, BND, XEDGE, S, J>(p, c, y - 2 * J, a0, a1, g, h);
         }
         x0 = g; x1 = h;   // (g, h) left the sub-step and flows on; (a0, a1) now waits in stage J
         if constexpr (J + 1 < S)
-            Stages<T, POT, BND, XEDGE, S, J + 1>::run(p, c, y, cs, nst, slotb, W, u, x0, x1);
+            Stages<T, PM, BND, XEDGE, S, J + 1>::run(p, c, y, cs, nst, slotb, W, u, x0, x1);
     }
 };
 
-template <typename T, int S, bool POT, int BND, int MINB>
+template <typename T, int S, int PM, int BND, int MINB>
 __global__ void __launch_bounds__(kWarps * 32, MINB)
 stream_kernel(const StreamParams<T> p) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     // BND: 0 = closed on both axes, 1 = periodic on both, 2 = periodic in x and closed in y (a row
     // slab of a larger lattice, paper_1208_2407_b200/slab.py)
     constexpr bool PERX = BND != 0, PERY = BND == 1;
+    constexpr bool POT = PM == 1;             // phase planes travel through the ring
     constexpr int R = POT ? S + 1 : 1;        // iterations a ring slot stays live after its arrival
     constexpr uint32_t ROWB = kStripSites * sizeof(T);
     constexpr int NROW = POT ? 8 : 4;         // re0 im0 re1 im1 [pr0 pi0 pr1 pi1]
@@ -253,6 +272,16 @@ stream_kernel(const StreamParams<T> p) {
     c.e.dn = !PERX && (xb + 4 == p.nx || xb + 4 == 0);
     c.ring = smem_u32(smem_raw) + warp * NST * SLOTB;
     c.lane_off = lane * 4 * sizeof(T);
+    if (PM == 2) {
+        // the lane's four columns (wrapped when periodic; 1 + 0i on ghost columns, which hold zeros)
+        const int xw = PERX ? wrap_index(xb, p.nx) : xb;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const bool ok = PERX || (xb >= 0 && xb < p.nx);
+            c.pxr[i] = ok ? __ldg(p.px_re + xw + i) : T(1);
+            c.pxi[i] = ok ? __ldg(p.px_im + xw + i) : T(0);
+        }
+    }
     const uint32_t bars = smem_u32(smem_raw) + kWarps * NST * SLOTB + warp * NST * 8;
     const bool store_ok = (4 * lane >= p.halo) && (4 * lane < kStripSites - p.halo) && (xb < p.nx);
 
@@ -367,7 +396,7 @@ stream_kernel(const StreamParams<T> p) {
                     zero_row(x0);
                     zero_row(x1);
                 }
-                Stages<T, POT, BND, XEDGE, S, 0>::run(p, c, y, cs, NST, SLOTB, W, U, x0, x1);
+                Stages<T, PM, BND, XEDGE, S, 0>::run(p, c, y, cs, NST, SLOTB, W, U, x0, x1);
                 if (it >= 2 * S && store_ok && y - 2 * S < y_out1) {
                     const int64_t off = (int64_t)(y - 2 * S) * p.nx + xb;
                     st4(p.dst_re + off, x0.re, p.out_scale);
@@ -388,17 +417,17 @@ stream_kernel(const StreamParams<T> p) {
     else run(std::false_type{});
 }
 
-template <typename T, int S, bool POT, int BND>
+template <typename T, int S, int PM, int BND>
 int launch(const StreamParams<T>& p, cudaStream_t st) {
-    constexpr uint32_t SLOTB = (POT ? 8 : 4) * kStripSites * sizeof(T);
+    constexpr uint32_t SLOTB = (PM == 1 ? 8 : 4) * kStripSites * sizeof(T);
     const size_t smem = (size_t)kWarps * p.nst * (SLOTB + 8);
-    // register budget: 4 blocks/SM (128 regs) for fp32 up to S = 4, 3 (168) beyond; 3 or 2 (255)
-    // for fp64
+    // register budget: the ring (64 KB per block) admits 3 blocks per SM anyway, so fp32 gets 168
+    // registers from S = 3 on (128 below); fp64 3 or 2 blocks (255)
 #ifndef TS_MINB_F32
-#define TS_MINB_F32 (S <= 4 ? 4 : 3)
+#define TS_MINB_F32 (S <= 2 ? 4 : 3)
 #endif
     constexpr int MINB = sizeof(T) == 4 ? TS_MINB_F32 : (S <= 2 ? 3 : 2);
-    auto kern = stream_kernel<T, S, POT, BND, MINB>;
+    auto kern = stream_kernel<T, S, PM, BND, MINB>;
     static size_t configured = 0;    // per instantiation
     if (smem > configured) {
         TS_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -412,32 +441,41 @@ int launch(const StreamParams<T>& p, cudaStream_t st) {
     return TS_OK;
 }
 
-template <typename T, int S, bool POT>
+template <typename T, int S, int PM>
 int launch_b(const StreamParams<T>& p, int bnd, cudaStream_t st) {
-    if (bnd == 1) return launch<T, S, POT, 1>(p, st);
-    if (bnd == 2) return launch<T, S, POT, 2>(p, st);
-    return launch<T, S, POT, 0>(p, st);
+    if (bnd == 1) return launch<T, S, PM, 1>(p, st);
+    if (bnd == 2) return launch<T, S, PM, 2>(p, st);
+    return launch<T, S, PM, 0>(p, st);
 }
 
 template <typename T, int S>
-int launch_s(const StreamParams<T>& p, bool pot, int bnd, cudaStream_t st) {
-    return pot ? launch_b<T, S, true>(p, bnd, st) : launch_b<T, S, false>(p, bnd, st);
+int launch_s(const StreamParams<T>& p, int pm, int bnd, cudaStream_t st) {
+    if (pm == 1) return launch_b<T, S, 1>(p, bnd, st);
+    if (pm == 2) return launch_b<T, S, 2>(p, bnd, st);
+    return launch_b<T, S, 0>(p, bnd, st);
 }
 
 template <typename T>
 int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T* dst_im,
-           const StepCoef* subs, const T* pot, int S, int seg_rows, int nst, cudaStream_t st) {
+           const StepCoef* subs, const Phase& ph, int S, int seg_rows, int nst, cudaStream_t st) {
     StreamParams<T> p;
     p.src_re = src_re; p.src_im = src_im; p.dst_re = dst_re; p.dst_im = dst_im;
+    const T* pot = ph.mode == 1 ? (const T*)ph.planes : nullptr;
     p.pot_re = pot;
     p.pot_im = pot ? pot + L.nx * L.ny : nullptr;
+    p.px_re = p.px_im = p.py_re = p.py_im = nullptr;
+    if (ph.mode == 2) {
+        p.px_re = (const T*)ph.px; p.px_im = p.px_re + L.nx;
+        p.py_re = (const T*)ph.py; p.py_im = p.py_re + L.ny;
+    }
+    const bool any = ph.mode != 0;        // the 6-sweeps-and-P stage, as opposed to the regrouped one
     p.nx = (int)L.nx; p.ny = (int)L.ny;
     p.halo = (2 * S + 3) / 4 * 4;
     p.wi = kStripSites - 2 * p.halo;
     p.n_strips = (int)((L.nx + p.wi - 1) / p.wi);
     p.seg_rows = seg_rows;
     const int live = pot ? S + 1 : 1;
-    if (nst <= 0) nst = stream_default_slots(L, S, pot != nullptr);
+    if (nst <= 0) nst = stream_default_slots(L, S, pot != nullptr);   // separable: as without
     if (nst < live + 1) nst = live + 1;
     const size_t slotb = (size_t)(pot ? 8 : 4) * kStripSites * sizeof(T);
     while (nst > live + 1 && (size_t)kWarps * nst * (slotb + 8) > 227u * 1024u) --nst;
@@ -464,7 +502,7 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
     }
     for (int j = 0; j < S; ++j) {
         const StepCoef& v = subs[j];
-        if (pot) {
+        if (any) {
             // Xo, Yo at the half angle, each twice per sub-step
             p.to[j] = (T)(v.b_h / v.a_h);
             p.sec_o[j] = (T)(1.0 / v.a_h);
@@ -480,14 +518,14 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
     p.out_scale = (T)scale;
     const int per = L.periodic_x ? (L.periodic_y ? 1 : 2) : 0;
     switch (S) {
-        case 1: return launch_s<T, 1>(p, pot != nullptr, per, st);
-        case 2: return launch_s<T, 2>(p, pot != nullptr, per, st);
-        case 3: return launch_s<T, 3>(p, pot != nullptr, per, st);
-        case 4: return launch_s<T, 4>(p, pot != nullptr, per, st);
+        case 1: return launch_s<T, 1>(p, ph.mode, per, st);
+        case 2: return launch_s<T, 2>(p, ph.mode, per, st);
+        case 3: return launch_s<T, 3>(p, ph.mode, per, st);
+        case 4: return launch_s<T, 4>(p, ph.mode, per, st);
     }
     // deeper temporal blocking only where the ALU budget allows it: fp32 without a potential
     if constexpr (sizeof(T) == 4) {
-        if (!pot) {
+        if (!any) {
             if (S == 5) return launch_b<T, 5, false>(p, per, st);
             if (S == 6) return launch_b<T, 6, false>(p, per, st);
         }
@@ -508,6 +546,12 @@ int stream_max_steps(const LatticeDesc& L, bool pot) {
     return (L.dtype == TS_F32 && !pot) ? 6 : 4;
 }
 
+int stream_default_steps_sep(const LatticeDesc& L) {
+    // no phase rows in the ring: the occupancy of the potential-free kernel, the arithmetic of the
+    // 6-sweeps-and-P stage (probe r1e)
+    return L.dtype == TS_F32 ? 4 : 3;
+}
+
 int stream_default_slots(const LatticeDesc& L, int S, bool pot) {
     // measured on B200 (profiles/r1b_probe.txt): 8 row-pair slots per warp keep ~7 iterations in
     // flight for fp32 without a potential (64 KB per block, 3 blocks per SM); with a potential a
@@ -517,7 +561,7 @@ int stream_default_slots(const LatticeDesc& L, int S, bool pot) {
 }
 
 int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
-                void* dst_im, const StepCoef* subs, const void* pot, int S, int seg_rows, int nst,
+                void* dst_im, const StepCoef* subs, const Phase& ph, int S, int seg_rows, int nst,
                 cudaStream_t st) {
     if (seg_rows <= 0 || seg_rows % 2) {
         set_error("stream_pass: seg_rows must be positive and even");
@@ -525,9 +569,9 @@ int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, vo
     }
     if (L.dtype == TS_F32)
         return pass_t<float>(L, (const float*)src_re, (const float*)src_im, (float*)dst_re,
-                             (float*)dst_im, subs, (const float*)pot, S, seg_rows, nst, st);
+                             (float*)dst_im, subs, ph, S, seg_rows, nst, st);
     return pass_t<double>(L, (const double*)src_re, (const double*)src_im, (double*)dst_re,
-                          (double*)dst_im, subs, (const double*)pot, S, seg_rows, nst, st);
+                          (double*)dst_im, subs, ph, S, seg_rows, nst, st);
 }
 
 }  // namespace ts

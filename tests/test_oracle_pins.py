@@ -315,3 +315,17 @@ def test_evolve_xy_with_equal_boundaries_is_evolve():
     oracle.evolve(re, im, *coeffs(0.2), periodic=True, n_steps=3)
     oracle.evolve_xy(r2, i2, *coeffs(0.2), periodic_x=True, periodic_y=True, n_steps=3)
     assert np.array_equal(re, r2) and np.array_equal(im, i2)
+
+
+# --- separable potential (harmonic trap: V = Vx + Vy) --------------------------------------------
+def test_evolve_sep_is_evolve_with_the_sum_potential():
+    nx, ny, theta = 10, 8, 0.23
+    rng = np.random.default_rng(3)
+    Vx, Vy = rng.uniform(-2, 2, nx), rng.uniform(-2, 2, ny)
+    re, im = rand_state(ny, nx, 6)
+    r2, i2 = re.copy(), im.copy()
+    V = Vy[:, None] + Vx[None, :]
+    oracle.evolve(re, im, *coeffs(theta), pot=(np.cos(V), -np.sin(V)), periodic=True, n_steps=4)
+    oracle.evolve_sep(r2, i2, *coeffs(theta), (np.cos(Vx), -np.sin(Vx)), (np.cos(Vy), -np.sin(Vy)),
+                      periodic=True, n_steps=4)
+    assert np.abs(re - r2).max() < 1e-14 and np.abs(im - i2).max() < 1e-14
