@@ -156,7 +156,10 @@ __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const Str
             // factors sit in registers; ghost rows are zero, so any finite factor will do there
             constexpr bool PERY = BND == 1;
             int ylo = yj - 1, yhi = yj;
-            if (PERY) { ylo = wrap_index(ylo, p.ny); yhi = wrap_index(yhi, p.ny); }
+            if (PERY) {   // |offset| < ny: one conditional add each way, no loop
+                ylo += ylo < 0 ? p.ny : 0;  ylo -= ylo >= p.ny ? p.ny : 0;
+                yhi += yhi < 0 ? p.ny : 0;  yhi -= yhi >= p.ny ? p.ny : 0;
+            }
             else { ylo = min(max(ylo, 0), p.ny - 1); yhi = min(max(yhi, 0), p.ny - 1); }
             sep_phase_row(h, c.pxr, c.pxi, __ldg(p.py_re + ylo), __ldg(p.py_im + ylo));
             sep_phase_row(a0, c.pxr, c.pxi, __ldg(p.py_re + yhi), __ldg(p.py_im + yhi));
@@ -549,7 +552,7 @@ int stream_max_steps(const LatticeDesc& L, bool pot) {
 int stream_default_steps_sep(const LatticeDesc& L) {
     // no phase rows in the ring: the occupancy of the potential-free kernel, the arithmetic of the
     // 6-sweeps-and-P stage (probe r1e)
-    return L.dtype == TS_F32 ? 4 : 3;
+    return L.dtype == TS_F32 ? 4 : 4;
 }
 
 int stream_default_slots(const LatticeDesc& L, int S, bool pot) {
