@@ -184,6 +184,13 @@ def run_gpu(args):
     eb = 4 if cfg.dtype == "f32" else 8
     re, im, _ = inputs.device_state(cfg, dev)
     pot = inputs.device_pot(cfg, dev)
+    sep = None
+    if args.sep:
+        if not cfg.has_pot:
+            raise SystemExit("--sep needs a config with a potential (C3, C5)")
+        sx, sy = inputs.sep_pot(cfg)
+        sep = (torch.from_numpy(sx).to(dev), torch.from_numpy(sy).to(dev))
+        pot = None
     plan = Plan(cfg.nx, cfg.ny, tdt, cfg.boundary)
     if args.fuse_steps:
         plan.set_option("fuse_steps", args.fuse_steps)
@@ -197,9 +204,15 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    def evolve_once():
+        if sep is not None:
+            plan.evolve_sep(re, im, *c, sep[0], sep[1], n_steps=cfg.n_steps, stream=stream)
+        else:
+            plan.evolve(re, im, *c, pot_phase=pot, n_steps=cfg.n_steps, stream=stream)
+
     n0 = plan.norm(re, im)
     for _ in range(args.warmup):
-        plan.evolve(re, im, *c, pot_phase=pot, n_steps=cfg.n_steps, stream=stream)
+        evolve_once()
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
@@ -210,7 +223,7 @@ def run_gpu(args):
     t0 = time.time()
     e0.record(stream)
     for _ in range(args.steps):
-        plan.evolve(re, im, *c, pot_phase=pot, n_steps=cfg.n_steps, stream=stream)
+        evolve_once()
     e1.record(stream)
     barrier()
     t1 = time.time()
@@ -233,14 +246,28 @@ def run_gpu(args):
     if pot is not None:
         hpot = torch.empty(pot.shape, dtype=tdt, pin_memory=True)
         hpot.copy_(pot)
-    del re, im
-    torch.cuda.empty_cache()
     e2e_reps = max(1, min(args.steps, 3))
-    plan.evolve_host(hre, him, *c, pot_phase=hpot, n_steps=cfg.n_steps)    # warm (allocations)
+    if sep is None:
+        del re, im
+        torch.cuda.empty_cache()
+        e2e_call = lambda: plan.evolve_host(hre, him, *c, pot_phase=hpot, n_steps=cfg.n_steps)
+        e2e_api = "ts_evolve_host (pinned host planes)"
+    else:
+        # separable entry: the state and the two phase vectors go up, the state comes back
+        hsx = sep[0].cpu().pin_memory(); hsy = sep[1].cpu().pin_memory()
+
+        def e2e_call():
+            re.copy_(hre, non_blocking=True); im.copy_(him, non_blocking=True)
+            sep[0].copy_(hsx, non_blocking=True); sep[1].copy_(hsy, non_blocking=True)
+            plan.evolve_sep(re, im, *c, sep[0], sep[1], n_steps=cfg.n_steps, stream=stream)
+            hre.copy_(re, non_blocking=True); him.copy_(im, non_blocking=True)
+            torch.cuda.synchronize()
+        e2e_api = "Plan.evolve_sep between pinned-host copies of the state and the phase vectors"
+    e2e_call()    # warm (allocations)
     barrier()
     t = time.perf_counter()
     for _ in range(e2e_reps):
-        plan.evolve_host(hre, him, *c, pot_phase=hpot, n_steps=cfg.n_steps)
+        e2e_call()
     barrier()
     e2e_s = (time.perf_counter() - t) / e2e_reps
     if dist is not None:
@@ -249,6 +276,8 @@ def run_gpu(args):
         e2e_s = float(tt.item())
     e2e_val = world * cfg.sites * cfg.n_steps / e2e_s
     h2d = (2 + (2 if pot is not None else 0)) * cfg.sites * eb
+    if sep is not None:
+        h2d += 2 * (cfg.nx + cfg.ny) * eb
     d2h = 2 * cfg.sites * eb
 
     if rank != 0:
@@ -257,7 +286,7 @@ def run_gpu(args):
     S = max(1, info["fuse_steps"])
     passes = max(1, info["passes"])
     # algorithmic bytes of one fused launch: read + write both planes once (+ phase planes once)
-    bytes_per_launch = cfg.sites * (4 * eb + (2 * eb if cfg.has_pot else 0))
+    bytes_per_launch = cfg.sites * (4 * eb + (2 * eb if (cfg.has_pot and sep is None) else 0))
     launch_ms = ms / (args.steps * passes)
     achieved = bytes_per_launch / (launch_ms * 1e-3) / 1e9
     traffic = None
@@ -272,7 +301,9 @@ def run_gpu(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
-        "config": {"workload": workload_text(cfg), "fuse_steps": S, "passes_per_call": passes,
+        "config": {"workload": workload_text(cfg) + (" (separable factors, ts_evolve_sep)"
+                                                     if sep is not None else ""),
+                   "fuse_steps": S, "passes_per_call": passes,
                    "seg_rows": info["seg_rows"], "fused": info["fused"],
                    "parallelism": "replicas only (no sharding of one lattice)",
                    "l2": "state (2 planes x 2 buffers) far larger than the 126 MB L2; no flush",
@@ -280,7 +311,7 @@ def run_gpu(args):
         "clocks": clocks,
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3,
-                "api": "ts_evolve_host (pinned host planes)"},
+                "api": e2e_api},
         "gpu_launches": info["launches"] * args.steps,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": traffic,
@@ -420,6 +451,8 @@ def main():
     ap.add_argument("--slabs", type=int, default=0,
                     help="N = 1: cut the lattice into this many slabs on the one GPU")
     ap.add_argument("--exchange-every", type=int, default=0, help="steps between halo exchanges")
+    ap.add_argument("--sep", action="store_true",
+                    help="C3/C5: pass the harmonic potential as separable factors (ts_evolve_sep)")
     ap.add_argument("--cpu-budget", type=float, default=1.5e9,
                     help="site-steps of oracle work in the cpu_baseline leg")
     args = ap.parse_args()

@@ -283,7 +283,11 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
             return fail(TS_EUNSUPPORTED, "fuse_steps > 4 needs the TMA ring kernel, fp32, no potential");
         S = s_max;
     }
-    const int seg = plan->opt_seg ? (int)plan->opt_seg : ts::fused_default_seg_rows(L, S);
+    // resident blocks per SM of the kernel that will run: the ring with phase planes is twice as
+    // large; fp64 pipelines beyond S = 2 take 255 registers
+    const bool planes = any_pot && !(any_sep && use_stream);
+    const int bpsm = (planes || (L.dtype == TS_F64 && S > 2)) ? 2 : 3;
+    const int seg = plan->opt_seg ? (int)plan->opt_seg : ts::fused_default_seg_rows(L, S, bpsm);
     plan->info_variant = use_stream ? 2 : 1;
     void* cur_re = psi_re; void* cur_im = psi_im;
     void* nxt_re = plan->scratch_re; void* nxt_im = plan->scratch_im;

@@ -257,18 +257,24 @@ bool fused_supported(const LatticeDesc& L, const StepCoef& c) {
     return fused_shape_ok(L, c) && L.periodic_x == L.periodic_y;
 }
 
-int fused_default_seg_rows(const LatticeDesc& L, int S) {
-    // One warp per (strip, segment); a segment recomputes 2S warm-up row pairs, so its cost is
-    // seg/2 + 2S iterations.  With W = strips * segments warps and room for ~12 warps on each of
-    // 148 SMs, time ~ max(W, 1776) * (seg/2 + 2S): longer segments win until the grid no longer
-    // fills the machine, so aim at one wave (probes r1d: 4096^2 best at ~92 rows, 16384^2 at
-    // 256 for S <= 4 and 512 beyond, 1024^2 at the lower clamp).
+int fused_default_seg_rows(const LatticeDesc& L, int S, int blocks_per_sm) {
+    // One warp per (strip, segment), 4 strips per block; a segment recomputes 2S warm-up row pairs,
+    // so its cost is seg/2 + 2S iterations: longer segments win until the grid no longer fills the
+    // machine.  Pick the number of waves the cap on the segment height allows (256 rows, 512 for
+    // S >= 5: probes r1d), then the segment count that fills those waves and no more -- a grid of
+    // 1.1 waves costs two (4096^2: 490 blocks on 444 slots ran at 60 % of the 16384^2 rate).
     const int halo = (2 * S + 3) / 4 * 4;
     const int64_t strips = (L.nx + (kStripSites - 2 * halo) - 1) / (kStripSites - 2 * halo);
-    const int64_t want = 148 * 12;
-    int64_t r = L.ny * strips / want;
-    r -= r % 2;
+    const int64_t blocks_x = (strips + 3) / 4;
+    const int64_t slots = 148 * (int64_t)(blocks_per_sm > 0 ? blocks_per_sm : 3);
     const int64_t cap = S >= 5 ? 512 : 256;
+    const int64_t min_segs = (L.ny + cap - 1) / cap;
+    int64_t waves = (min_segs * blocks_x + slots - 1) / slots;
+    if (waves < 1) waves = 1;
+    int64_t segs = waves * slots / blocks_x;
+    if (segs < 1) segs = 1;
+    int64_t r = (L.ny + segs - 1) / segs;
+    r += r % 2;
     if (r > cap) r = cap;
     if (r < 8) r = 8;     // small lattices: parallelism over warm-up redundancy
     if (r > L.ny) r = L.ny;

@@ -54,7 +54,7 @@ bool fused_supported(const LatticeDesc& L, const StepCoef& c);  // + same bounda
 int fused_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
                void* dst_im, const StepCoef& c, const void* pot, int S, int seg_rows,
                cudaStream_t st);
-int fused_default_seg_rows(const LatticeDesc& L, int S);
+int fused_default_seg_rows(const LatticeDesc& L, int S, int blocks_per_sm = 3);
 
 // ---- fused streaming path v2 (ts_stream.cu): TMA bulk copies into a per-warp smem ring ---------
 bool stream_supported(const LatticeDesc& L, const StepCoef& c);

@@ -254,3 +254,16 @@ def device_pot(cfg: Config, device, chunk_rows: int = 2048):
         pot[0, y0:y1] = torch.cos(V).to(dt)
         pot[1, y0:y1] = (-torch.sin(V)).to(dt)
     return pot
+
+
+def sep_pot(cfg: Config):
+    """The harmonic potential of the recipe as SEPARABLE phase factors (host numpy, config dtype):
+    V = 0.5 w^2 (x-cx)^2 + 0.5 w^2 (y-cy)^2, so exp(-i V) = px(x) * py(y);
+    returns (phase_x [2][nx], phase_y [2][ny]) = (cos, -sin) of the two 1-D terms, or None."""
+    if not cfg.has_pot:
+        return None
+    dt = np_dtype(cfg)
+    vx = 0.5 * cfg.omega ** 2 * (np.arange(cfg.nx, dtype=np.float64) - cfg.cx) ** 2
+    vy = 0.5 * cfg.omega ** 2 * (np.arange(cfg.ny, dtype=np.float64) - cfg.cy) ** 2
+    return (np.stack([np.cos(vx), -np.sin(vx)]).astype(dt),
+            np.stack([np.cos(vy), -np.sin(vy)]).astype(dt))
