@@ -217,6 +217,13 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
         can_v1 = can_v1 && ts::fused_supported(L, c);
         can_stream = can_stream && ts::stream_supported(L, c);
     }
+    // sub-steps chained inside a pass merge their adjacent half sweeps: that angle, too, must
+    // stay away from 90 degrees for the tangent form
+    for (int k = 0; k < period && period > 1; ++k) {
+        const ts::StepCoef& u = pat[k].c;
+        const ts::StepCoef& v = pat[(k + 1) % period].c;
+        if (u.a_h * v.a_h - u.b_h * v.b_h <= 0.25) can_v1 = can_stream = false;
+    }
     const bool can_fuse = can_v1 || can_stream;
     int rc = check_device(plan);
     if (rc != TS_OK) return rc;

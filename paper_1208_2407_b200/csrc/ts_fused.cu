@@ -250,7 +250,8 @@ bool fused_shape_ok(const LatticeDesc& L, const StepCoef& c) {
     // 128-bit row accesses need nx % 4 == 0; the row-pair pipeline needs even ny; the tangent
     // form needs cos well away from zero; 32-bit row/column indices inside the kernel.
     return L.nx % 4 == 0 && L.ny % 2 == 0 && L.nx >= 4 && L.ny >= 2 &&
-           L.nx < (1 << 30) && L.ny < (1 << 30) && c.a_h > 0.25 && c.a_f > 0.25;
+           L.nx < (1 << 30) && L.ny < (1 << 30) && c.a_h > 0.25 && c.a_f > 0.25 &&
+           c.a_h * c.a_h - c.b_h * c.b_h > 0.25;   // two half sweeps merged into one
 }
 
 bool fused_supported(const LatticeDesc& L, const StepCoef& c) {

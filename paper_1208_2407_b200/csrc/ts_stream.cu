@@ -47,8 +47,11 @@ struct StreamParams {
     // sub-step to sub-step: Eq. 4 chains U2 with three different time fractions)
     T te[TS_MAX_FUSE + 1];   // even sweeps: te[0] opening half sweep, te[j] the merged sweep between
                              // sub-steps j-1 and j (half + half angle), te[S] the closing half sweep
-    T to[TS_MAX_FUSE];       // odd sweeps of sub-step j: full angle without potential, half with
-    T sec_o[TS_MAX_FUSE];    // 1 / cos of that odd sweep (unpaired sites at closed edges)
+    T to[TS_MAX_FUSE];       // Y-odd sweep of sub-step j: the caller's full-angle coefficients
+                             // without potential; with one, every odd sweep at the half angle
+    T sec_o[TS_MAX_FUSE];    // 1 / cos of that sweep (unpaired sites at closed edges)
+    T tox[TS_MAX_FUSE];      // X-odd sweep without potential: the two half sweeps Xo(h) Xo(h) that
+    T sec_ox[TS_MAX_FUSE];   // regrouping brings together, composed from the HALF coefficients
     T out_scale;             // product of all deferred cosines of the pass
 };
 
@@ -203,7 +206,7 @@ __device__ __forceinline__ void stream_stage_nopot(const StreamParams<T>& p,
                                                    Row4<T>& a1, Row4<T>& g, Row4<T>& h) {
     constexpr bool LAST = J == S - 1;
     xe(a0, p.te[J]); xe(a1, p.te[J]);
-    xo<T, XEDGE>(a0, p.to[J], p.sec_o[J], c.e); xo<T, XEDGE>(a1, p.to[J], p.sec_o[J], c.e);
+    xo<T, XEDGE>(a0, p.tox[J], p.sec_ox[J], c.e); xo<T, XEDGE>(a1, p.tox[J], p.sec_ox[J], c.e);
     if (LAST) { xe(a0, p.te[S]); xe(a1, p.te[S]); }
     ypair(a0, a1, p.te[J]);
     // closed lattice: the vertical-odd pair (yj-1, yj) does not exist at yj = 0 and yj = ny; the
@@ -511,13 +514,20 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
             p.sec_o[j] = (T)(1.0 / v.a_h);
             scale *= pow(v.a_h, 4);
         } else {
-            // Xo and Yo at the full angle, once each
+            // Yo once with the caller's full-angle coefficients (the "full middle sweep"); Xo once
+            // by twice the half angle: the regrouped form of Xo(h) ... Xo(h)
             p.to[j] = (T)(v.b_f / v.a_f);
             p.sec_o[j] = (T)(1.0 / v.a_f);
-            scale *= v.a_f * v.a_f;
+            const double c2 = v.a_h * v.a_h - v.b_h * v.b_h, s2 = 2.0 * v.a_h * v.b_h;
+            p.tox[j] = (T)(s2 / c2);
+            p.sec_ox[j] = (T)(1.0 / c2);
+            scale *= v.a_f * c2;
         }
     }
-    for (int j = S; j < TS_MAX_FUSE; ++j) { p.to[j] = T(0); p.sec_o[j] = T(1); p.te[j + 1] = T(0); }
+    for (int j = 0; j < TS_MAX_FUSE; ++j) {
+        if (any || j >= S) { p.tox[j] = T(0); p.sec_ox[j] = T(1); }
+        if (j >= S) { p.to[j] = T(0); p.sec_o[j] = T(1); p.te[j + 1] = T(0); }
+    }
     p.out_scale = (T)scale;
     const int per = L.periodic_x ? (L.periodic_y ? 1 : 2) : 0;
     switch (S) {

@@ -95,6 +95,29 @@ def test_generic_path(nx, ny, boundary, with_pot, dtype):
     assert info["fused"] == 0 and info["launches"] <= 6 * (9 if with_pot else 7)
 
 
+@pytest.mark.parametrize("boundary", ["closed", "periodic"])
+@pytest.mark.parametrize("fuse", [1, 3, 6])
+def test_full_angle_coefficients_need_not_be_twice_the_half_angle(boundary, fuse):
+    # ts.h: (a_full, b_full) belong to the middle sweep only.  The regrouped kernel merges half
+    # sweeps, and must build those merged angles from the HALF coefficients, not from a_full.
+    nx, ny, n = 252, 66, 7
+    cfg = G.make_cfg(nx, ny, "f64", boundary, 0.3, n)
+    re, im, _ = G.random_inputs(nx, ny, "f64", 321, False)
+    c = (math.cos(0.15), math.sin(0.15), math.cos(0.47), math.sin(0.47))   # full != 2 * half
+    got_re, got_im, info = G.gpu_evolve(cfg, re, im, None, n_steps=n, path=2, fuse=min(fuse, 4),
+                                        seg_rows=16, coeffs=c)
+    want_re, want_im = G.oracle_evolve(cfg, re, im, None, n_steps=n, coeffs=c)
+    err, _ = G.errors(cfg, got_re, got_im, want_re, want_im)
+    assert err < 1e-13, (err, info)
+    cfg32 = G.make_cfg(nx, ny, "f32", boundary, 0.3, n)
+    re32, im32, _ = G.random_inputs(nx, ny, "f32", 322, False)
+    got_re, got_im, info = G.gpu_evolve(cfg32, re32, im32, None, n_steps=n, path=2, fuse=fuse,
+                                        seg_rows=16, coeffs=c)
+    want_re, want_im = G.oracle_evolve(cfg32, re32, im32, None, n_steps=n, coeffs=c)
+    err, _ = G.errors(cfg32, got_re, got_im, want_re, want_im)
+    assert err < 2e-5, (err, info)
+
+
 def test_auto_path_picks_generic_for_unaligned_shapes():
     cfg = G.make_cfg(130, 31, "f32", "closed", 0.2, 4)
     re, im, pot = G.random_inputs(130, 31, "f32", 5, True)
