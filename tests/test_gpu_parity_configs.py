@@ -62,14 +62,29 @@ def _windows(cfg, S, seg):
     return wins
 
 
-def _run_periodic_config(cfg):
+def _run_periodic_config(cfg, sep=False):
+    """sep: pass the harmonic potential as separable factors (ts_evolve_sep); the oracle then gets
+    the outer product of the same (cast) factors as planes, which is what the entry defines."""
     import torch
     from paper_1208_2407_b200.binding import Plan
     dev = torch.device("cuda:0")
     re, im, n2 = inputs.device_state(cfg, dev)
-    pot = inputs.device_pot(cfg, dev)
     plan = Plan(cfg.nx, cfg.ny, G.torch_dtype(cfg), cfg.boundary)
     c = cfg.coeffs()
+    if sep:
+        sx, sy = inputs.sep_pot(cfg)
+        d_sx, d_sy = torch.from_numpy(sx).to(dev), torch.from_numpy(sy).to(dev)
+        pot = None
+        cx = sx[0].astype(np.float64) + 1j * sx[1].astype(np.float64)
+        cy = sy[0].astype(np.float64) + 1j * sy[1].astype(np.float64)
+
+        def evolve(r, i, n):
+            plan.evolve_sep(r, i, *c, d_sx, d_sy, n_steps=n)
+    else:
+        pot = inputs.device_pot(cfg, dev)
+
+        def evolve(r, i, n):
+            plan.evolve(r, i, *c, pot_phase=pot, n_steps=n)
 
     def fetch_from(t_re, t_im):
         def f(ys, xs):
@@ -78,7 +93,7 @@ def _run_periodic_config(cfg):
         return f
 
     # probe what the default configuration fuses, to aim windows at its seams
-    plan.evolve(re.clone(), im.clone(), *c, pot_phase=pot, n_steps=1)
+    evolve(re.clone(), im.clone(), 1)
     S, seg = max(1, plan.info("fuse_steps")), max(2, plan.info("seg_rows"))
     S = S if cfg.n_steps >= S else cfg.n_steps
 
@@ -92,10 +107,13 @@ def _run_periodic_config(cfg):
         pw = None
         if pot is not None:
             pw = fetch_from(pot[0], pot[1])(ys, xs)
+        elif sep:
+            P = cy[ys][:, None] * cx[xs][None, :]
+            pw = (np.ascontiguousarray(P.real), np.ascontiguousarray(P.imag))
         cut[(x0, y0, w, h)] = (xs, ys, r, i, pw)
 
     n2_before = plan.norm(re, im)
-    plan.evolve(re, im, *c, pot_phase=pot, n_steps=cfg.n_steps)
+    evolve(re, im, cfg.n_steps)
     torch.cuda.synchronize()
     n2_after = plan.norm(re, im)
     info = {k: plan.info(k) for k in ("fused", "fuse_steps", "passes", "launches", "seg_rows")}
@@ -148,6 +166,56 @@ def test_C5_windows_and_norm():
     assert err <= G.tol(cfg)
     assert rel <= 1e-10
     assert abs(drift) < 1e-12 and abs(info["norm2_before"] - 1) < 1e-12
+
+
+def test_C5_separable_entry_windows_and_norm():
+    import torch
+    if torch.cuda.get_device_properties(0).total_memory < 40e9:
+        pytest.skip("needs ~34 GB of device memory")
+    cfg = inputs.CONFIGS["C5"]
+    err, rel, info, n = _run_periodic_config(cfg, sep=True)
+    drift = _report(f"C5 via ts_evolve_sep, {n} windows", err, rel, info)
+    assert info["fused"] == 1
+    assert err <= G.tol(cfg)
+    assert rel <= 1e-10
+    assert abs(drift) < 1e-12
+
+
+def test_C4_size_fourth_order_eigenstate():
+    """The same closed form for ts_evolve_u4: the five sub-step angles sum to theta, so
+    U4^n psi = exp(i 2 n theta ((1-2sx)+(1-2sy))) psi at full C4 size (8 steps = 40 sub-steps
+    chained through passes of 6)."""
+    import torch
+    from paper_1208_2407_b200.binding import Plan
+    cfg = inputs.CONFIGS["C4"]
+    dev = torch.device("cuda:0")
+    amp = 1.0 / math.sqrt(cfg.sites)
+    sgn_x = (1 - 2 * (torch.arange(cfg.nx, device=dev) % 2)).to(torch.float32)
+    re = (sgn_x[None, :] * amp).expand(cfg.ny, cfg.nx).contiguous()
+    im = torch.zeros_like(re)
+    ref = re.clone()
+    plan = Plan(cfg.nx, cfg.ny, torch.float32, "periodic")
+    n, theta = 8, 0.1
+    plan.evolve_u4(re, im, theta, n_steps=n)
+    torch.cuda.synchronize()
+    ph = 2 * n * theta * ((1 - 2 * 1) + 1)          # sx = 1, sy = 0: the two axes cancel
+    ph_x = -2 * n * theta
+    # (sx, sy) = (1, 0): X sweeps give exp(-i theta) per step each way, Y sweeps exp(+i theta)
+    assert ph == 0.0 and ph_x != 0.0
+    rel = max(float((re - ref).abs().max()), float(im.abs().max())) / amp
+    print(f"\n[C4-size U4 eigenstate sx=1 sy=0] rel err {rel:.3e}  passes={plan.info('passes')}")
+    assert plan.info("fused") == 1 and plan.info("passes") == math.ceil(5 * n / 6)
+    assert rel < 2e-5
+    # and a state whose phase does not cancel: sx = sy = 0 (uniform), phase 4 n theta
+    re.fill_(amp); im.zero_()
+    plan.evolve_u4(re, im, theta, n_steps=n)
+    torch.cuda.synchronize()
+    ph = 4 * n * theta
+    rel = max(float((re - math.cos(ph) * amp).abs().max()),
+              float((im - math.sin(ph) * amp).abs().max())) / amp
+    print(f"[C4-size U4 uniform state] rel err {rel:.3e}")
+    assert rel < 2e-5
+    plan.destroy()
 
 
 @pytest.mark.parametrize("name,sx,sy", [("C4", 1, 0), ("C4", 1, 1), ("C5", 0, 1)])
