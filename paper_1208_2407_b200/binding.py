@@ -13,7 +13,7 @@ TS_MAX_FUSE = 6
 _LIB_PATH = Path(__file__).resolve().parent / "libts.so"
 _lib = None
 
-SYMBOLS = ["ts_plan_create", "ts_plan_create_xy", "ts_evolve", "ts_evolve_u4", "ts_evolve_sep",
+SYMBOLS = ["ts_plan_create", "ts_plan_create_xy", "ts_evolve", "ts_evolve_u4", "ts_evolve_sep", "ts_slab_pass",
            "ts_norm", "ts_evolve_host", "ts_plan_set_option",
            "ts_plan_get_info", "ts_plan_destroy", "ts_last_error"]
 
@@ -43,6 +43,9 @@ def lib():
         L.ts_evolve_u4.restype = i32
         L.ts_evolve_sep.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp, vp, i64, vp]
         L.ts_evolve_sep.restype = i32
+        L.ts_slab_pass.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, vp, vp, i64, dbl, dbl, dbl, dbl,
+                                   i32, vp]
+        L.ts_slab_pass.restype = i32
         L.ts_norm.argtypes = [vp, vp, vp, ctypes.POINTER(dbl), vp]
         L.ts_norm.restype = i32
         L.ts_evolve_host.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp, i64]
@@ -165,6 +168,28 @@ class Plan:
                                    b_full, ctypes.c_void_p(phase_x.data_ptr()),
                                    ctypes.c_void_p(phase_y.data_ptr()), int(n_steps),
                                    _stream_handle(stream)))
+
+    def slab_pass(self, src, dst, up, dn, a_half, b_half, a_full, b_full, n_sub, stream=None):
+        """ts_slab_pass: src, dst = (re, im) CUDA planes of this slab; up, dn = (re, im) planes of
+        the neighbours (any row count >= 2*n_sub; may be peer-GPU memory) or None at a closed edge."""
+        self._planes(src[0], src[1]); self._planes(dst[0], dst[1])
+
+        def nb(t):
+            if t is None:
+                return None, None, 0
+            re, im = t
+            if re.dtype != self.dtype or re.shape[1] != self.nx or re.shape != im.shape or \
+                    not (re.is_contiguous() and im.is_contiguous() and re.is_cuda):
+                raise ValueError("neighbour planes must be contiguous CUDA tensors [rows][nx]")
+            return ctypes.c_void_p(re.data_ptr()), ctypes.c_void_p(im.data_ptr()), re.shape[0]
+        ur, ui, un = nb(up)
+        dr, di, dn_rows = nb(dn)
+        _check(lib().ts_slab_pass(self._h, ctypes.c_void_p(src[0].data_ptr()),
+                                  ctypes.c_void_p(src[1].data_ptr()),
+                                  ctypes.c_void_p(dst[0].data_ptr()),
+                                  ctypes.c_void_p(dst[1].data_ptr()), ur, ui, un, dr, di, dn_rows,
+                                  a_half, b_half, a_full, b_full, int(n_sub),
+                                  _stream_handle(stream)))
 
     def evolve_host(self, psi_re, psi_im, a_half, b_half, a_full, b_full, pot_phase=None,
                     n_steps=1):

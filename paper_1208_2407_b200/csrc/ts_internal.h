@@ -31,6 +31,16 @@ struct Phase {
     const void* py;
 };
 
+// Neighbours of a row slab (ts_slab_pass): their SOURCE planes of this pass and their row counts.
+struct Peers {
+    const void* up_re;
+    const void* up_im;
+    int64_t up_rows;
+    const void* dn_re;
+    const void* dn_im;
+    int64_t dn_rows;
+};
+
 struct LatticeDesc {
     int64_t nx, ny;
     int dtype;      // TS_F32 / TS_F64
@@ -65,7 +75,7 @@ int stream_default_slots(const LatticeDesc& L, int S, bool pot);
 // (fourth-order step, Eq. 4) but share one potential-phase array.
 int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
                 void* dst_im, const StepCoef* subs, const Phase& ph, int S, int seg_rows, int nst,
-                cudaStream_t st);
+                cudaStream_t st, const Peers* peers = nullptr);
 // pot[2][ny][nx] <- px (x) py: the separable factors written out for paths that take planes
 int expand_separable(const LatticeDesc& L, const void* px, const void* py, void* pot,
                      cudaStream_t st);

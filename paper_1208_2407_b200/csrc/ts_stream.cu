@@ -40,6 +40,15 @@ struct StreamParams {
     const T* px_im;
     const T* py_re;
     const T* py_im;
+    // row slab with peer halos (ts_slab_pass): rows above row 0 / below row ny-1 are read from
+    // the neighbours' source planes (their last up_rows / first dn_rows rows; possibly another
+    // GPU's memory over NVLink).  NULL = no neighbour: a real closed edge (or plain lattice).
+    const T* up_re;
+    const T* up_im;
+    const T* dn_re;
+    const T* dn_im;
+    int up_rows, dn_rows;
+    int edge_top, edge_bot;   // closed in y: row 0 / row ny-1 is a lattice edge (not a cut)
     int nx, ny;
     int n_strips, wi, halo, seg_rows;
     int nst;        // ring slots per warp
@@ -148,7 +157,7 @@ __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const Str
     ypair(a0, a1, p.te[J]);
     // closed lattice: the vertical-odd pair (yj-1, yj) does not exist at yj = 0 and yj = ny; the
     // ghost row is zero and stays zero (coupling 0), the real row takes 1/a per omitted sweep
-    const bool yedge = XEDGE && (yj == 0 || yj == p.ny);
+    const bool yedge = XEDGE && ((yj == 0 && p.edge_top) || (yj == p.ny && p.edge_bot));
     const T t_yo = yedge ? T(0) : th;
     ypair(h, a0, t_yo);
     {
@@ -211,7 +220,7 @@ __device__ __forceinline__ void stream_stage_nopot(const StreamParams<T>& p,
     ypair(a0, a1, p.te[J]);
     // closed lattice: the vertical-odd pair (yj-1, yj) does not exist at yj = 0 and yj = ny; the
     // real row of the two takes 1/a instead (the ghost row is zero and stays zero)
-    const bool yedge = XEDGE && (yj == 0 || yj == p.ny);
+    const bool yedge = XEDGE && ((yj == 0 && p.edge_top) || (yj == p.ny && p.edge_bot));
     const T t_yo = yedge ? T(0) : p.to[J];
     ypair(h, a0, t_yo);
     if (XEDGE) { const T sy = yedge ? p.sec_o[J] : T(1); scale_row(h, sy); scale_row(a0, sy); }
@@ -330,17 +339,32 @@ stream_kernel(const StreamParams<T> p) {
 
     // fetch the next row pair into ring slot `slot` (one elected lane issues all copies)
     auto issue = [&](int slot) {
-        const bool rowok = PERY ? true : (fy >= 0 && fy < p.ny);
+        // where the row pair lives: own planes, or a neighbour's (slab with peer halos)
+        bool rowok = true;
+        const T* b_re = p.src_re;
+        const T* b_im = p.src_im;
+        int64_t off = foff;
+        if (!PERY) {
+            if (fy < 0) {
+                rowok = p.up_re != nullptr && fy + p.up_rows >= 0;
+                b_re = p.up_re; b_im = p.up_im;
+                off = (int64_t)(fy + p.up_rows) * p.nx;
+            } else if (fy >= p.ny) {
+                rowok = p.dn_re != nullptr && fy - p.ny + 2 <= p.dn_rows;
+                b_re = p.dn_re; b_im = p.dn_im;
+                off = (int64_t)(fy - p.ny) * p.nx;
+            }
+        }
         if (leader) {
             const uint32_t bar = bars + 8 * slot;
             if (rowok) {
                 mbar_arrive_expect_tx(bar, slot_tx);
                 const uint32_t dst = c.ring + slot * SLOTB;
-                const T* planes[8] = {p.src_re, p.src_im, p.src_re, p.src_im,
+                const T* planes[8] = {b_re, b_im, b_re, b_im,
                                       p.pot_re, p.pot_im, p.pot_re, p.pot_im};
 #pragma unroll
                 for (int r = 0; r < NROW; ++r) {
-                    const T* row = planes[r] + foff + ((r >> 1) & 1) * p.nx;
+                    const T* row = planes[r] + (r < 4 ? off : foff) + ((r >> 1) & 1) * p.nx;
                     bulk_g2s(dst + r * ROWB + dst_a, row + gx_a, bytes_a, bar);
                     if (bytes_b) bulk_g2s(dst + r * ROWB + dst_b, row, bytes_b, bar);
                 }
@@ -390,7 +414,8 @@ stream_kernel(const StreamParams<T> p) {
                 if (it + DIST < n_iter) issue(rs);
                 mbar_wait(bars + 8 * cs, cph);
                 const int y = y_in0 + 2 * it;
-                const bool rowok = !XEDGE || (y >= 0 && y < p.ny && c.xvalid);
+                const bool rowok = !XEDGE || (c.xvalid && (y >= 0 || !p.edge_top) &&
+                                              (y < p.ny || !p.edge_bot));
                 Row4<T> x0, x1;
                 if (rowok) {
                     const uint32_t base = c.ring + cs * SLOTB + c.lane_off;
@@ -418,7 +443,8 @@ stream_kernel(const StreamParams<T> p) {
         half(std::integral_constant<int, 1>{});
     }
     };   // run
-    const bool edge = c.xedge || (!PERY && (y_in0 < 0 || y_in0 + 2 * n_iter >= p.ny));
+    const bool edge = c.xedge || (!PERY && ((y_in0 < 0 && p.edge_top) ||
+                                            (y_in0 + 2 * n_iter >= p.ny && p.edge_bot)));
     if (edge) run(std::true_type{});
     else run(std::false_type{});
 }
@@ -463,8 +489,18 @@ int launch_s(const StreamParams<T>& p, int pm, int bnd, cudaStream_t st) {
 
 template <typename T>
 int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T* dst_im,
-           const StepCoef* subs, const Phase& ph, int S, int seg_rows, int nst, cudaStream_t st) {
+           const StepCoef* subs, const Phase& ph, int S, int seg_rows, int nst, cudaStream_t st,
+           const Peers* peers) {
     StreamParams<T> p;
+    p.up_re = p.up_im = p.dn_re = p.dn_im = nullptr;
+    p.up_rows = p.dn_rows = 0;
+    if (peers) {
+        p.up_re = (const T*)peers->up_re; p.up_im = (const T*)peers->up_im;
+        p.dn_re = (const T*)peers->dn_re; p.dn_im = (const T*)peers->dn_im;
+        p.up_rows = (int)peers->up_rows; p.dn_rows = (int)peers->dn_rows;
+    }
+    p.edge_top = p.up_re == nullptr;
+    p.edge_bot = p.dn_re == nullptr;
     p.src_re = src_re; p.src_im = src_im; p.dst_re = dst_re; p.dst_im = dst_im;
     const T* pot = ph.mode == 1 ? (const T*)ph.planes : nullptr;
     p.pot_re = pot;
@@ -575,16 +611,16 @@ int stream_default_slots(const LatticeDesc& L, int S, bool pot) {
 
 int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
                 void* dst_im, const StepCoef* subs, const Phase& ph, int S, int seg_rows, int nst,
-                cudaStream_t st) {
+                cudaStream_t st, const Peers* peers) {
     if (seg_rows <= 0 || seg_rows % 2) {
         set_error("stream_pass: seg_rows must be positive and even");
         return TS_EINVAL;
     }
     if (L.dtype == TS_F32)
         return pass_t<float>(L, (const float*)src_re, (const float*)src_im, (float*)dst_re,
-                             (float*)dst_im, subs, ph, S, seg_rows, nst, st);
+                             (float*)dst_im, subs, ph, S, seg_rows, nst, st, peers);
     return pass_t<double>(L, (const double*)src_re, (const double*)src_im, (double*)dst_re,
-                          (double*)dst_im, subs, ph, S, seg_rows, nst, st);
+                          (double*)dst_im, subs, ph, S, seg_rows, nst, st, peers);
 }
 
 }  // namespace ts

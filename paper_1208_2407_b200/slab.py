@@ -280,3 +280,158 @@ class LocalGroup:
     def destroy(self):
         for s in self.slabs:
             s.destroy()
+
+
+# ---- fused halo path: ts_slab_pass reads the neighbours' boundary rows in place ------------------
+def max_fused_steps(dtype) -> int:
+    """Deepest pass ts_slab_pass takes (csrc/ts_stream.cu::stream_max_steps, no potential)."""
+    import torch
+    return 6 if dtype == torch.float32 else 4
+
+
+class PeerSlab:
+    """One rank's slab for the fused path: its own rows only, in two buffers that ping-pong; there
+    is NO halo storage and no exchange step -- `ts_slab_pass` fetches the rows beyond the slab
+    straight from the neighbours' source buffers (same GPU here, a peer GPU's mapped memory in
+    `PeerRank`).  buffers: optional [2][2][rows >= own][nx] tensor to live in (symmetric memory)."""
+
+    def __init__(self, nx, ny, dtype, boundary, rank, world, device, buffers=None):
+        import torch
+        from .binding import Plan
+        self.nx, self.ny, self.dtype, self.boundary = int(nx), int(ny), dtype, boundary
+        self.rank, self.world = int(rank), int(world)
+        self.r0, self.r1 = partition_rows(self.ny, self.world)[self.rank]
+        self.own = self.r1 - self.r0
+        # on a periodic lattice every rank has both neighbours -- a single rank is its own
+        per = boundary == "periodic"
+        self.nb = Neighbours((rank - 1) % world, (rank + 1) % world) if per else \
+            neighbours(self.rank, self.world, False)
+        if buffers is None:
+            buffers = torch.zeros((2, 2, self.own, self.nx), dtype=dtype, device=device)
+        self.buffers = buffers
+        self.cur = 0
+        self.plan = Plan(self.nx, self.own, dtype, boundary, "closed")
+        self.norm_plan = self.plan
+
+    def planes(self, which):
+        """(re, im) views of buffer `which` restricted to the own rows."""
+        b = self.buffers[which]
+        return b[0, :self.own], b[1, :self.own]
+
+    def set_state(self, re_own, im_own):
+        re, im = self.planes(self.cur)
+        re.copy_(re_own); im.copy_(im_own)
+
+    def launch_pass(self, up_src, dn_src, coeffs, n_sub, stream=None):
+        """dst <- U2^n_sub src with the neighbours' CURRENT planes as halos; does not flip."""
+        self.plan.slab_pass(self.planes(self.cur), self.planes(1 - self.cur), up_src, dn_src,
+                            *coeffs, n_sub, stream=stream)
+
+    def flip(self):
+        self.cur = 1 - self.cur
+
+    def norm_local(self) -> float:
+        re, im = self.planes(self.cur)
+        return self.plan.norm(re, im)
+
+    def destroy(self):
+        self.plan.destroy()
+
+
+class PeerGroup:
+    """All ranks of the fused path in one process on one device.  One stream orders the passes:
+    every slab's pass k reads only buffers written by pass k-1, so launching the slabs one after
+    the other and flipping all of them afterwards is the barrier."""
+
+    def __init__(self, nx, ny, dtype, boundary, world, device):
+        self.slabs = [PeerSlab(nx, ny, dtype, boundary, r, world, device) for r in range(world)]
+        self.S = max_fused_steps(dtype)
+        smallest = min(s.own for s in self.slabs)
+        if smallest < 2:
+            raise ValueError("slabs need at least one row pair")
+        # a pass consumes 2 rows per sub-step from each neighbour
+        self.S = max(1, min(self.S, smallest // 2))
+
+    def scatter(self, re, im):
+        for s in self.slabs:
+            s.set_state(re[s.r0:s.r1], im[s.r0:s.r1])
+
+    def gather(self, re, im):
+        for s in self.slabs:
+            r, i = s.planes(s.cur)
+            re[s.r0:s.r1].copy_(r); im[s.r0:s.r1].copy_(i)
+
+    def evolve(self, coeffs, n_steps):
+        left = int(n_steps)
+        while left > 0:
+            k = min(self.S, left)
+            for s in self.slabs:
+                up = self.slabs[s.nb.up].planes(self.slabs[s.nb.up].cur) if s.nb.up is not None \
+                    else None
+                dn = self.slabs[s.nb.down].planes(self.slabs[s.nb.down].cur) \
+                    if s.nb.down is not None else None
+                s.launch_pass(up, dn, coeffs, k)
+            for s in self.slabs:
+                s.flip()
+            left -= k
+
+    def norm(self) -> float:
+        return sum(s.norm_local() for s in self.slabs)
+
+    def destroy(self):
+        for s in self.slabs:
+            s.destroy()
+
+
+class PeerRank:
+    """The fused path with one process per GPU: the two buffers of every rank live in symmetric
+    memory (torch.distributed._symmetric_memory), so each rank holds mapped views of its
+    neighbours' buffers and `ts_slab_pass` reads their boundary rows over NVLink inside the
+    kernel's own bulk copies.  Between passes: one device-side barrier over the group
+    (`handle.barrier`), which orders "everybody finished writing pass k" before "anybody reads
+    pass k".  NOT RUN on hardware in this round (needs >= 2 GPUs); the single-process twin
+    `PeerGroup` runs the identical kernel path with neighbours on the same device."""
+
+    def __init__(self, nx, ny, dtype, boundary, group=None):
+        import torch
+        import torch.distributed as dist
+        import torch.distributed._symmetric_memory as symm
+        self.group = group if group is not None else dist.group.WORLD
+        rank, world = dist.get_rank(self.group), dist.get_world_size(self.group)
+        dev = torch.device("cuda", torch.cuda.current_device())
+        rows = max(b - a for a, b in partition_rows(ny, world))      # same shape on every rank
+        self.shape = (2, 2, rows, int(nx))
+        buf = symm.empty(self.shape, dtype=dtype, device=dev)
+        buf.zero_()
+        self.handle = symm.rendezvous(buf, self.group)
+        self.slab = PeerSlab(nx, ny, dtype, boundary, rank, world, dev, buffers=buf)
+        parts = partition_rows(ny, world)
+        self.peer_own = [b - a for a, b in parts]
+        self.peer_buf = {}
+        for r in {self.slab.nb.up, self.slab.nb.down} - {None}:
+            self.peer_buf[r] = buf if r == rank else \
+                self.handle.get_buffer(r, self.shape, dtype, 0)
+        self.S = max(1, min(max_fused_steps(dtype), min(self.peer_own) // 2))
+        self.comm = DistComm(self.group)
+
+    def _peer_planes(self, r, which):
+        if r is None:
+            return None
+        b = self.peer_buf[r][which]
+        n = self.peer_own[r]
+        return b[0, :n], b[1, :n]
+
+    def evolve(self, coeffs, n_steps):
+        s = self.slab
+        left = int(n_steps)
+        while left > 0:
+            k = min(self.S, left)
+            self.handle.barrier(channel=0)          # every rank's previous pass is complete
+            s.launch_pass(self._peer_planes(s.nb.up, s.cur), self._peer_planes(s.nb.down, s.cur),
+                          coeffs, k)
+            s.flip()                                # all ranks flip in step: same parity everywhere
+            left -= k
+        self.handle.barrier(channel=0)
+
+    def norm(self) -> float:
+        return self.comm.all_reduce_sum(self.slab.norm_local())

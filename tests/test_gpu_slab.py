@@ -81,3 +81,53 @@ def test_slab_decomposition_matches_undivided_oracle(world, boundary, with_pot, 
     assert abs(n0 / oracle.norm2(re.astype(np.float64), im.astype(np.float64)) - 1) < 1e-6
     assert abs(n1 / n0 - 1) < (1e-4 if dtype == "f32" else 1e-12)
     g.destroy()
+
+
+@pytest.mark.parametrize("world", [1, 2, 3])
+@pytest.mark.parametrize("boundary", ["closed", "periodic"])
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_fused_peer_halo_path_matches_undivided_oracle(world, boundary, dtype):
+    # ts_slab_pass: no halo storage, no exchange step -- the kernel reads the neighbours' rows
+    import torch
+    from paper_1208_2407_b200 import slab
+    dev = torch.device("cuda:0")
+    nx, ny, n = 380, 132, 17                # 17 steps = passes of 6, 6, 5 (fp32) / 4, 4, 4, 4, 1
+    re, im, _ = G.random_inputs(nx, ny, dtype, 500 + world, False)
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    g = slab.PeerGroup(nx, ny, tdt, boundary, world, dev)
+    g.scatter(torch.from_numpy(re).to(dev), torch.from_numpy(im).to(dev))
+    n0 = g.norm()
+    g.evolve(coeffs(0.3), n)
+    out_re = torch.empty((ny, nx), dtype=tdt, device=dev); out_im = torch.empty_like(out_re)
+    g.gather(out_re, out_im)
+    torch.cuda.synchronize()
+    n1 = g.norm()
+    wre, wim = re.astype(np.float64), im.astype(np.float64)
+    oracle.evolve(wre, wim, *coeffs(0.3), periodic=boundary == "periodic", n_steps=n)
+    err = max(np.abs(out_re.cpu().numpy() - wre).max(), np.abs(out_im.cpu().numpy() - wim).max())
+    assert err <= TIGHT[dtype] * 3, err
+    assert abs(n1 / n0 - 1) < (1e-4 if dtype == "f32" else 1e-12)
+    g.destroy()
+
+
+def test_slab_pass_argument_errors():
+    import torch
+    from paper_1208_2407_b200.binding import Plan, TsError
+    dev = torch.device("cuda:0")
+    plan = Plan(128, 16, torch.float32, "periodic", "closed")
+    a = (torch.zeros((16, 128), device=dev), torch.zeros((16, 128), device=dev))
+    b = (torch.zeros((16, 128), device=dev), torch.zeros((16, 128), device=dev))
+    short = (torch.zeros((4, 128), device=dev), torch.zeros((4, 128), device=dev))
+    c = coeffs(0.1)
+    with pytest.raises(TsError):
+        plan.slab_pass(a, a, None, None, *c, 2)              # in place
+    with pytest.raises(TsError):
+        plan.slab_pass(a, b, short, None, *c, 3)             # neighbour shorter than the halo
+    with pytest.raises(TsError):
+        plan.slab_pass(a, b, None, None, *c, 7)              # deeper than the kernel goes
+    plan.slab_pass(a, b, short, short, *c, 2)
+    plan.destroy()
+    per = Plan(128, 16, torch.float32, "periodic")
+    with pytest.raises(TsError):
+        per.slab_pass(a, b, None, None, *c, 1)               # slab plans are closed in y
+    per.destroy()
