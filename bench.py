@@ -355,7 +355,25 @@ def run_gpu_slab(args):
     pot = inputs.device_pot(cfg, dev)
     k = args.exchange_every or slab.default_steps_per_exchange(tdt, pot is not None)
     c = cfg.coeffs()
-    if world > 1:
+    fused_halo = args.slab_mode == "peer"
+    if fused_halo and pot is not None:
+        raise SystemExit("--slab-mode peer (ts_slab_pass) has no potential: use C1, C2 or C4")
+    if fused_halo and world > 1:
+        # one process per GPU, buffers in symmetric memory, halos read over NVLink in the kernel
+        obj = slab.PeerRank(cfg.nx, cfg.ny * world, tdt, cfg.boundary)
+        obj.slab.set_state(re, im)
+        evolve = lambda: obj.evolve(c, cfg.n_steps)
+        norm = obj.norm
+        plans = [obj.slab.plan]
+        n_slabs, halo, k = world, 2 * obj.S, obj.S
+    elif fused_halo:
+        obj = slab.PeerGroup(cfg.nx, cfg.ny, tdt, cfg.boundary, max(1, args.slabs), dev)
+        obj.scatter(re, im)
+        evolve = lambda: obj.evolve(c, cfg.n_steps)
+        norm = obj.norm
+        plans = [s.plan for s in obj.slabs]
+        n_slabs, halo, k = len(obj.slabs), 2 * obj.S, obj.S
+    elif world > 1:
         comm = slab.DistComm()
         obj = slab.Slab(cfg.nx, cfg.ny * world, tdt, cfg.boundary, rank, world, k, device=dev)
         obj.set_state(re, im)
@@ -405,7 +423,7 @@ def run_gpu_slab(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
     n1 = norm()
-    S = max(1, plans[0].info("fuse_steps"))
+    S = obj.S if fused_halo else max(1, plans[0].info("fuse_steps"))
     periods = -(-cfg.n_steps // k)
     launches = sum(p.info("launches") for p in plans) * periods      # last period may be shorter
     sites = cfg.sites * world
@@ -420,8 +438,12 @@ def run_gpu_slab(args):
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
         "config": {"workload": workload_text(cfg) + (f", stacked {world}x in y" if world > 1 else ""),
-                   "parallelism": f"row slabs x{n_slabs}, halo {halo} rows exchanged every {k} steps"
-                                  + (" over NCCL" if world > 1 else " (one GPU, slabs stepped in turn)"),
+                   "parallelism": (f"row slabs x{n_slabs}, halo {halo} rows "
+                                   + ("read from the neighbours inside the kernel (ts_slab_pass) "
+                                      f"every pass of {k} steps" if fused_halo else
+                                      f"exchanged every {k} steps")
+                                   + ((" over NVLink peer memory" if fused_halo else " over NCCL")
+                                      if world > 1 else " (one GPU, slabs stepped in turn)")),
                    "fuse_steps": S, "norm2_before": n0, "norm_drift": n1 / n0 - 1,
                    "l2": "state far larger than the 126 MB L2; no flush"},
         "clocks": clocks, "gpu_launches": launches * args.steps,
@@ -450,6 +472,9 @@ def main():
                          "cut into row slabs with NCCL halo exchange")
     ap.add_argument("--slabs", type=int, default=0,
                     help="N = 1: cut the lattice into this many slabs on the one GPU")
+    ap.add_argument("--slab-mode", default="exchange", choices=["exchange", "peer"],
+                    help="slabs: halo exchange step + ts_evolve, or ts_slab_pass reading the "
+                         "neighbours' rows inside the kernel (no potential)")
     ap.add_argument("--exchange-every", type=int, default=0, help="steps between halo exchanges")
     ap.add_argument("--sep", action="store_true",
                     help="C3/C5: pass the harmonic potential as separable factors (ts_evolve_sep)")
@@ -460,7 +485,7 @@ def main():
         args.warmup = 3
     if args.impl == "reference":
         return run_reference(args)
-    if args.decomp == "slab" or args.slabs > 1:
+    if args.decomp == "slab" or args.slabs > 1 or args.slab_mode == "peer":
         return run_gpu_slab(args)
     return run_gpu(args)
 
