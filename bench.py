@@ -356,19 +356,29 @@ def run_gpu_slab(args):
     k = args.exchange_every or slab.default_steps_per_exchange(tdt, pot is not None)
     c = cfg.coeffs()
     fused_halo = args.slab_mode == "peer"
+    sep = None
     if fused_halo and pot is not None:
-        raise SystemExit("--slab-mode peer (ts_slab_pass) has no potential: use C1, C2 or C4")
+        # ts_slab_pass takes the potential as separable factors (the harmonic trap is separable)
+        stacked = inputs.scaled(cfg, cfg.nx, cfg.ny * world) if world > 1 else cfg
+        sx, sy = inputs.sep_pot(stacked)
+        sep = (torch.from_numpy(sx).to(dev), torch.from_numpy(sy).to(dev))
+        pot = None
     if fused_halo and world > 1:
         # one process per GPU, buffers in symmetric memory, halos read over NVLink in the kernel
         obj = slab.PeerRank(cfg.nx, cfg.ny * world, tdt, cfg.boundary)
         obj.slab.set_state(re, im)
+        if sep is not None:
+            obj.set_separable_potential(*sep)
         evolve = lambda: obj.evolve(c, cfg.n_steps)
         norm = obj.norm
         plans = [obj.slab.plan]
         n_slabs, halo, k = world, 2 * obj.S, obj.S
     elif fused_halo:
         obj = slab.PeerGroup(cfg.nx, cfg.ny, tdt, cfg.boundary, max(1, args.slabs), dev)
-        obj.scatter(re, im)
+        if sep is not None:
+            obj.scatter(re, im, *sep)
+        else:
+            obj.scatter(re, im)
         evolve = lambda: obj.evolve(c, cfg.n_steps)
         norm = obj.norm
         plans = [s.plan for s in obj.slabs]
@@ -431,7 +441,7 @@ def run_gpu_slab(args):
     if rank != 0:
         return 0
     peak, peak_src = load_peaks()
-    bytes_per_site_step = (4 * eb + (2 * eb if cfg.has_pot else 0)) / S
+    bytes_per_site_step = (4 * eb + (2 * eb if (cfg.has_pot and not fused_halo) else 0)) / S
     achieved = value / world * bytes_per_site_step / 1e9
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

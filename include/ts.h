@@ -120,27 +120,34 @@ int ts_evolve_sep(ts_plan* plan, void* psi_re, void* psi_im,
 
 /*
  * ts_slab_pass -- ONE fused pass over a row slab of a larger lattice, halos read in place from
- * the neighbouring slabs: dst <- U2^n_sub src on the plan's nx x ny rows, where the rows above
- * row 0 are the LAST up_rows rows of (up_re, up_im) and the rows below row ny-1 are the FIRST
- * dn_rows rows of (dn_re, dn_im) -- the neighbours' source planes of this same pass, in this GPU's
- * memory or mapped from a peer GPU (NVLink).  This is the compute step and the halo "exchange"
- * of the distributed solver in one kernel: the bulk copies that feed the
- * pipeline simply take the rows beyond the slab from the neighbour's address.  No potential.
+ * the neighbouring slabs: dst <- U2(c[n_sub-1]) ... U2(c[0]) src on the plan's nx x ny rows, where
+ * the rows above row 0 are the LAST up_rows rows of (up_re, up_im) and the rows below row ny-1
+ * are the FIRST dn_rows rows of (dn_re, dn_im) -- the neighbours' source planes of this same
+ * pass, in this GPU's memory or mapped from a peer GPU (NVLink).  This is the compute step and the
+ * halo "exchange" of the distributed solver in one kernel: the bulk copies
+ * that feed the pipeline simply take the rows beyond the slab from the neighbour's address.
  *   plan        from ts_plan_create_xy(nx, ny_slab, dtype, boundary_x, TS_CLOSED); ny_slab even.
  *   src, dst    DEVICE planes of the slab, distinct (out of place; the caller ping-pongs).
  *   up_*, dn_*  neighbour planes (pitch nx) or NULL for a real closed edge of the lattice;
  *               up_rows, dn_rows even and >= 2*n_sub.
- *   n_sub       sub-steps fused in this pass: 1..6 (fp32), 1..4 (fp64).
+ *   coef        HOST table, n_sub rows of (a_half, b_half, a_full, b_full): the sub-steps of this
+ *               pass in order of application (equal rows: plain steps; the Eq. 4 pattern: U4).
+ *   n_sub       sub-steps fused in this pass: 1..6 (fp32 without potential), else 1..4.
+ *   phase_x, phase_y, y0, ny_global, periodic_y_global
+ *               both NULL: no potential.  Else the separable phase of ts_evolve_sep, phase_y
+ *               covering the GLOBAL lattice (2*ny_global elements); slab row y is global row
+ *               y0 + y (y0 even), and rows beyond the global lattice wrap if periodic_y_global.
  * The caller must make sure that the neighbours have finished writing their source planes
  * (i.e. the previous pass) before this pass starts, and do not overwrite them before it ends:
- * one barrier over the ranks between passes (paper_1208_2407_b200/slab.py::PeerGroup).
+ * one barrier over the ranks between passes (paper_1208_2407_b200/slab.py::PeerRank).
  * Errors: TS_EINVAL, TS_EUNSUPPORTED (shapes the TMA ring kernel does not take), TS_ECUDA.
  */
 int ts_slab_pass(ts_plan* plan, const void* src_re, const void* src_im, void* dst_re, void* dst_im,
                  const void* up_re, const void* up_im, int64_t up_rows,
                  const void* dn_re, const void* dn_im, int64_t dn_rows,
-                 double a_half, double b_half, double a_full, double b_full,
-                 int n_sub, void* cuda_stream);
+                 const double* coef, int n_sub,
+                 const void* phase_x, const void* phase_y, int64_t y0, int64_t ny_global,
+                 int periodic_y_global, void* cuda_stream);
 
 /*
  * ts_norm -- squared norm sum |psi|^2, accumulated in double for either dtype.

@@ -43,8 +43,8 @@ def lib():
         L.ts_evolve_u4.restype = i32
         L.ts_evolve_sep.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp, vp, i64, vp]
         L.ts_evolve_sep.restype = i32
-        L.ts_slab_pass.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, vp, vp, i64, dbl, dbl, dbl, dbl,
-                                   i32, vp]
+        L.ts_slab_pass.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, vp, vp, i64,
+                                   ctypes.POINTER(dbl), i32, vp, vp, i64, i64, i32, vp]
         L.ts_slab_pass.restype = i32
         L.ts_norm.argtypes = [vp, vp, vp, ctypes.POINTER(dbl), vp]
         L.ts_norm.restype = i32
@@ -169,9 +169,12 @@ class Plan:
                                    ctypes.c_void_p(phase_y.data_ptr()), int(n_steps),
                                    _stream_handle(stream)))
 
-    def slab_pass(self, src, dst, up, dn, a_half, b_half, a_full, b_full, n_sub, stream=None):
+    def slab_pass(self, src, dst, up, dn, coef, phase_x=None, phase_y=None, y0=0, ny_global=0,
+                  periodic_y_global=False, stream=None):
         """ts_slab_pass: src, dst = (re, im) CUDA planes of this slab; up, dn = (re, im) planes of
-        the neighbours (any row count >= 2*n_sub; may be peer-GPU memory) or None at a closed edge."""
+        the neighbours (any row count >= 2*n_sub; may be peer-GPU memory) or None at a closed edge;
+        coef = sequence of (a_half, b_half, a_full, b_full), one per fused sub-step; phase_x
+        [2][nx], phase_y [2][ny_global] = separable potential phase or None."""
         self._planes(src[0], src[1]); self._planes(dst[0], dst[1])
 
         def nb(t):
@@ -184,12 +187,22 @@ class Plan:
             return ctypes.c_void_p(re.data_ptr()), ctypes.c_void_p(im.data_ptr()), re.shape[0]
         ur, ui, un = nb(up)
         dr, di, dn_rows = nb(dn)
+        flat = [float(v) for row in coef for v in row]
+        n_sub = len(flat) // 4
+        table = (ctypes.c_double * len(flat))(*flat)
+        px = py = None
+        if phase_x is not None:
+            if phase_x.dtype != self.dtype or tuple(phase_x.shape) != (2, self.nx) or \
+                    phase_y.dtype != self.dtype or tuple(phase_y.shape) != (2, int(ny_global)) or \
+                    not (phase_x.is_contiguous() and phase_y.is_contiguous() and phase_x.is_cuda):
+                raise ValueError("phase_x [2][nx], phase_y [2][ny_global]: contiguous CUDA tensors")
+            px, py = ctypes.c_void_p(phase_x.data_ptr()), ctypes.c_void_p(phase_y.data_ptr())
         _check(lib().ts_slab_pass(self._h, ctypes.c_void_p(src[0].data_ptr()),
                                   ctypes.c_void_p(src[1].data_ptr()),
                                   ctypes.c_void_p(dst[0].data_ptr()),
                                   ctypes.c_void_p(dst[1].data_ptr()), ur, ui, un, dr, di, dn_rows,
-                                  a_half, b_half, a_full, b_full, int(n_sub),
-                                  _stream_handle(stream)))
+                                  table, n_sub, px, py, int(y0), int(ny_global),
+                                  int(bool(periodic_y_global)), _stream_handle(stream)))
 
     def evolve_host(self, psi_re, psi_im, a_half, b_half, a_full, b_full, pot_phase=None,
                     n_steps=1):

@@ -356,43 +356,60 @@ int ts_evolve_sep(ts_plan* plan, void* psi_re, void* psi_im, double a_half, doub
 
 int ts_slab_pass(ts_plan* plan, const void* src_re, const void* src_im, void* dst_re,
                  void* dst_im, const void* up_re, const void* up_im, int64_t up_rows,
-                 const void* dn_re, const void* dn_im, int64_t dn_rows, double a_half,
-                 double b_half, double a_full, double b_full, int n_sub, void* cuda_stream) {
+                 const void* dn_re, const void* dn_im, int64_t dn_rows, const double* coef,
+                 int n_sub, const void* phase_x, const void* phase_y, int64_t y0,
+                 int64_t ny_global, int periodic_y_global, void* cuda_stream) {
     if (!plan) return fail(TS_EINVAL, "NULL plan");
     if (!src_re || !src_im || !dst_re || !dst_im) return fail(TS_EINVAL, "NULL psi plane");
+    if (!coef) return fail(TS_EINVAL, "NULL coefficient table");
     if ((up_re == nullptr) != (up_im == nullptr) || (dn_re == nullptr) != (dn_im == nullptr))
         return fail(TS_EINVAL, "give both planes of a neighbour or neither");
+    if ((phase_x == nullptr) != (phase_y == nullptr))
+        return fail(TS_EINVAL, "give both separable phase vectors or neither");
     const ts::LatticeDesc& L = plan->L;
     if (L.periodic_y)
         return fail(TS_EINVAL, "a slab plan is closed in y (ts_plan_create_xy(.., bx, TS_CLOSED))");
     const size_t plane_bytes = (size_t)L.nx * (size_t)L.ny * plan->elem;
-    const void* ptrs[8] = {src_re, src_im, dst_re, dst_im, up_re, up_im, dn_re, dn_im};
+    const void* ptrs[10] = {src_re, src_im, dst_re, dst_im, up_re, up_im, dn_re, dn_im, phase_x,
+                            phase_y};
     for (const void* q : ptrs)
         if (q && !aligned16(q)) return fail(TS_EINVAL, "device pointers must be 16-byte aligned");
     if (overlap(src_re, dst_re, plane_bytes) || overlap(src_im, dst_im, plane_bytes) ||
         overlap(src_re, dst_im, plane_bytes) || overlap(src_im, dst_re, plane_bytes))
         return fail(TS_EINVAL, "ts_slab_pass works out of place: src and dst overlap");
-    if (!coef_ok(a_half, b_half) || !coef_ok(a_full, b_full))
-        return fail(TS_EINVAL, "coefficients must be finite with |a^2 + b^2 - 1| <= 1e-6");
-    const ts::StepCoef c{a_half, b_half, a_full, b_full};
-    if (!ts::stream_supported(L, c))
-        return fail(TS_EUNSUPPORTED, "ts_slab_pass runs on the TMA ring kernel only: nx >= 128, "
-                                     "nx % 4 == 0, even ny, cos(theta) > 0.25");
-    const int s_max = ts::stream_max_steps(L, false);
+    const bool sep = phase_x != nullptr;
+    const int s_max = ts::stream_max_steps(L, sep);
     if (n_sub < 1 || n_sub > s_max) return fail(TS_EINVAL, "n_sub out of range for this dtype");
+    ts::StepCoef subs[TS_MAX_FUSE];
+    for (int j = 0; j < n_sub; ++j) {
+        subs[j] = ts::StepCoef{coef[4 * j], coef[4 * j + 1], coef[4 * j + 2], coef[4 * j + 3]};
+        if (!coef_ok(subs[j].a_h, subs[j].b_h) || !coef_ok(subs[j].a_f, subs[j].b_f))
+            return fail(TS_EINVAL, "coefficients must be finite with |a^2 + b^2 - 1| <= 1e-6");
+        bool ok = ts::stream_supported(L, subs[j]);
+        if (ok && j > 0)   // the merged half sweeps between chained sub-steps
+            ok = subs[j - 1].a_h * subs[j].a_h - subs[j - 1].b_h * subs[j].b_h > 0.25;
+        if (!ok)
+            return fail(TS_EUNSUPPORTED, "ts_slab_pass runs on the TMA ring kernel only: nx >= 128, "
+                                         "nx % 4 == 0, even ny, cos of every sweep angle > 0.25");
+    }
     // the halo a pass consumes: 2 rows per sub-step from each neighbour
     if ((up_re && up_rows < 2 * n_sub) || (dn_re && dn_rows < 2 * n_sub))
         return fail(TS_EINVAL, "a neighbour has fewer than 2 * n_sub rows");
     if (up_rows % 2 || dn_rows % 2) return fail(TS_EINVAL, "neighbour row counts must be even");
+    ts::Phase ph{0, nullptr, nullptr, nullptr};
+    if (sep) {
+        if (ny_global < L.ny || y0 < 0 || y0 + L.ny > ny_global || y0 % 2)
+            return fail(TS_EINVAL, "the slab [y0, y0 + ny) must lie inside the global lattice, y0 even");
+        ph.mode = 2; ph.px = phase_x; ph.py = phase_y;
+        ph.py_off = y0; ph.py_n = ny_global; ph.py_wrap = periodic_y_global != 0;
+    }
     int rc = check_device(plan);
     if (rc != TS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
-    ts::StepCoef subs[TS_MAX_FUSE];
-    for (int j = 0; j < n_sub; ++j) subs[j] = c;
     const ts::Peers peers{up_re, up_im, up_rows, dn_re, dn_im, dn_rows};
     const int seg = plan->opt_seg ? (int)plan->opt_seg : ts::fused_default_seg_rows(L, n_sub, 3);
-    rc = ts::stream_pass(L, src_re, src_im, dst_re, dst_im, subs, ts::Phase{0, nullptr, nullptr, nullptr},
-                         n_sub, seg, (int)plan->opt_slots, st, &peers);
+    rc = ts::stream_pass(L, src_re, src_im, dst_re, dst_im, subs, ph, n_sub, seg,
+                         (int)plan->opt_slots, st, &peers);
     if (rc != TS_OK) return rc;
     plan->info_fused = 1; plan->info_fuse = n_sub; plan->info_passes = 1; plan->info_launches = 1;
     plan->info_seg = seg; plan->info_variant = 2;

@@ -29,6 +29,11 @@ struct Phase {
     const void* planes;
     const void* px;
     const void* py;
+    // separable phase of a row slab: py covers the GLOBAL lattice (py_n rows, py_n = 0: the plan's
+    // own ny), local row 0 is global row py_off, py_wrap = global lattice periodic in y
+    int64_t py_off = 0;
+    int64_t py_n = 0;
+    int py_wrap = 0;
 };
 
 // Neighbours of a row slab (ts_slab_pass): their SOURCE planes of this pass and their row counts.

@@ -49,6 +49,7 @@ struct StreamParams {
     const T* dn_im;
     int up_rows, dn_rows;
     int edge_top, edge_bot;   // closed in y: row 0 / row ny-1 is a lattice edge (not a cut)
+    int py_off, py_n, py_wrap;   // separable phase: global row of local row 0, global height, wrap
     int nx, ny;
     int n_strips, wi, halo, seg_rows;
     int nst;        // ring slots per warp
@@ -166,13 +167,14 @@ __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const Str
         if (PM == 2) {
             // separable: the row factors come through L1 (one address per warp), the column
             // factors sit in registers; ghost rows are zero, so any finite factor will do there
-            constexpr bool PERY = BND == 1;
-            int ylo = yj - 1, yhi = yj;
-            if (PERY) {   // |offset| < ny: one conditional add each way, no loop
-                ylo += ylo < 0 ? p.ny : 0;  ylo -= ylo >= p.ny ? p.ny : 0;
-                yhi += yhi < 0 ? p.ny : 0;  yhi -= yhi >= p.ny ? p.ny : 0;
+            // py is indexed by the GLOBAL row: py_off = first row of a slab (0 for a whole
+            // lattice), py_n = global height, py_wrap = the global lattice is periodic in y
+            int ylo = yj - 1 + p.py_off, yhi = yj + p.py_off;
+            if (p.py_wrap) {   // |excursion| < py_n: one conditional add each way, no loop
+                ylo += ylo < 0 ? p.py_n : 0;  ylo -= ylo >= p.py_n ? p.py_n : 0;
+                yhi += yhi < 0 ? p.py_n : 0;  yhi -= yhi >= p.py_n ? p.py_n : 0;
             }
-            else { ylo = min(max(ylo, 0), p.ny - 1); yhi = min(max(yhi, 0), p.ny - 1); }
+            else { ylo = min(max(ylo, 0), p.py_n - 1); yhi = min(max(yhi, 0), p.py_n - 1); }
             sep_phase_row(h, c.pxr, c.pxi, __ldg(p.py_re + ylo), __ldg(p.py_im + ylo));
             sep_phase_row(a0, c.pxr, c.pxi, __ldg(p.py_re + yhi), __ldg(p.py_im + yhi));
         } else {
@@ -506,9 +508,13 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
     p.pot_re = pot;
     p.pot_im = pot ? pot + L.nx * L.ny : nullptr;
     p.px_re = p.px_im = p.py_re = p.py_im = nullptr;
+    p.py_off = 0; p.py_n = (int)L.ny; p.py_wrap = L.periodic_y;
     if (ph.mode == 2) {
         p.px_re = (const T*)ph.px; p.px_im = p.px_re + L.nx;
-        p.py_re = (const T*)ph.py; p.py_im = p.py_re + L.ny;
+        const int64_t ny_g = ph.py_n > 0 ? ph.py_n : L.ny;
+        p.py_re = (const T*)ph.py; p.py_im = p.py_re + ny_g;
+        p.py_off = (int)ph.py_off; p.py_n = (int)ny_g;
+        p.py_wrap = ph.py_n > 0 ? ph.py_wrap : L.periodic_y;
     }
     const bool any = ph.mode != 0;        // the 6-sweeps-and-P stage, as opposed to the regrouped one
     p.nx = (int)L.nx; p.ny = (int)L.ny;

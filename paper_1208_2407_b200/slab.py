@@ -283,10 +283,32 @@ class LocalGroup:
 
 
 # ---- fused halo path: ts_slab_pass reads the neighbours' boundary rows in place ------------------
-def max_fused_steps(dtype) -> int:
-    """Deepest pass ts_slab_pass takes (csrc/ts_stream.cu::stream_max_steps, no potential)."""
+def max_fused_steps(dtype, with_pot: bool = False) -> int:
+    """Deepest pass ts_slab_pass takes (csrc/ts_stream.cu::stream_max_steps)."""
     import torch
-    return 6 if dtype == torch.float32 else 4
+    return 6 if (dtype == torch.float32 and not with_pot) else 4
+
+
+def step_coeffs(theta):
+    """(a_half, b_half, a_full, b_full) of one second-order step of angle theta."""
+    import math
+    return (math.cos(theta / 2), math.sin(theta / 2), math.cos(theta), math.sin(theta))
+
+
+def u4_pattern(theta):
+    """The five sub-steps of the fourth-order step, Eq. 4."""
+    p = 1.0 / (4.0 - 4.0 ** (1.0 / 3.0))
+    return [step_coeffs(f * theta) for f in (p, p, 1.0 - 4.0 * p, p, p)]
+
+
+def _passes(pattern, n_repeat, depth):
+    """Cut n_repeat repetitions of a sub-step pattern into passes of at most `depth` sub-steps."""
+    total = len(pattern) * int(n_repeat)
+    i = 0
+    while i < total:
+        k = min(depth, total - i)
+        yield [pattern[(i + j) % len(pattern)] for j in range(k)]
+        i += k
 
 
 class PeerSlab:
@@ -310,6 +332,7 @@ class PeerSlab:
             buffers = torch.zeros((2, 2, self.own, self.nx), dtype=dtype, device=device)
         self.buffers = buffers
         self.cur = 0
+        self.sep = None
         self.plan = Plan(self.nx, self.own, dtype, boundary, "closed")
         self.norm_plan = self.plan
 
@@ -322,10 +345,17 @@ class PeerSlab:
         re, im = self.planes(self.cur)
         re.copy_(re_own); im.copy_(im_own)
 
-    def launch_pass(self, up_src, dn_src, coeffs, n_sub, stream=None):
-        """dst <- U2^n_sub src with the neighbours' CURRENT planes as halos; does not flip."""
+    def set_separable_potential(self, phase_x, phase_y):
+        """phase_x [2][nx], phase_y [2][ny] over the GLOBAL lattice (every rank holds both)."""
+        self.sep = (phase_x, phase_y)
+
+    def launch_pass(self, up_src, dn_src, subs, stream=None):
+        """dst <- U2(subs[-1]) ... U2(subs[0]) src with the neighbours' CURRENT planes as halos;
+        does not flip."""
+        px, py = self.sep if self.sep is not None else (None, None)
         self.plan.slab_pass(self.planes(self.cur), self.planes(1 - self.cur), up_src, dn_src,
-                            *coeffs, n_sub, stream=stream)
+                            subs, px, py, self.r0, self.ny, self.boundary == "periodic",
+                            stream=stream)
 
     def flip(self):
         self.cur = 1 - self.cur
@@ -345,35 +375,45 @@ class PeerGroup:
 
     def __init__(self, nx, ny, dtype, boundary, world, device):
         self.slabs = [PeerSlab(nx, ny, dtype, boundary, r, world, device) for r in range(world)]
-        self.S = max_fused_steps(dtype)
-        smallest = min(s.own for s in self.slabs)
-        if smallest < 2:
+        self.dtype = dtype
+        self.smallest = min(s.own for s in self.slabs)
+        if self.smallest < 2:
             raise ValueError("slabs need at least one row pair")
-        # a pass consumes 2 rows per sub-step from each neighbour
-        self.S = max(1, min(self.S, smallest // 2))
+        self.S = self._depth(False)
 
-    def scatter(self, re, im):
+    def _depth(self, with_pot):
+        # a pass consumes 2 rows per sub-step from each neighbour
+        return max(1, min(max_fused_steps(self.dtype, with_pot), self.smallest // 2))
+
+    def scatter(self, re, im, phase_x=None, phase_y=None):
         for s in self.slabs:
             s.set_state(re[s.r0:s.r1], im[s.r0:s.r1])
+            if phase_x is not None:
+                s.set_separable_potential(phase_x, phase_y)
+        self.S = self._depth(phase_x is not None)
 
     def gather(self, re, im):
         for s in self.slabs:
             r, i = s.planes(s.cur)
             re[s.r0:s.r1].copy_(r); im[s.r0:s.r1].copy_(i)
 
-    def evolve(self, coeffs, n_steps):
-        left = int(n_steps)
-        while left > 0:
-            k = min(self.S, left)
+    def run(self, pattern, n_repeat):
+        """n_repeat repetitions of a list of sub-step coefficient tuples."""
+        for subs in _passes(pattern, n_repeat, self.S):
             for s in self.slabs:
                 up = self.slabs[s.nb.up].planes(self.slabs[s.nb.up].cur) if s.nb.up is not None \
                     else None
                 dn = self.slabs[s.nb.down].planes(self.slabs[s.nb.down].cur) \
                     if s.nb.down is not None else None
-                s.launch_pass(up, dn, coeffs, k)
+                s.launch_pass(up, dn, subs)
             for s in self.slabs:
                 s.flip()
-            left -= k
+
+    def evolve(self, coeffs, n_steps):
+        self.run([tuple(coeffs)], n_steps)
+
+    def evolve_u4(self, theta, n_steps):
+        self.run(u4_pattern(theta), n_steps)
 
     def norm(self) -> float:
         return sum(s.norm_local() for s in self.slabs)
@@ -411,8 +451,13 @@ class PeerRank:
         for r in {self.slab.nb.up, self.slab.nb.down} - {None}:
             self.peer_buf[r] = buf if r == rank else \
                 self.handle.get_buffer(r, self.shape, dtype, 0)
+        self.dtype = dtype
         self.S = max(1, min(max_fused_steps(dtype), min(self.peer_own) // 2))
         self.comm = DistComm(self.group)
+
+    def set_separable_potential(self, phase_x, phase_y):
+        self.slab.set_separable_potential(phase_x, phase_y)
+        self.S = max(1, min(max_fused_steps(self.dtype, True), min(self.peer_own) // 2))
 
     def _peer_planes(self, r, which):
         if r is None:
@@ -421,17 +466,20 @@ class PeerRank:
         n = self.peer_own[r]
         return b[0, :n], b[1, :n]
 
-    def evolve(self, coeffs, n_steps):
+    def run(self, pattern, n_repeat):
         s = self.slab
-        left = int(n_steps)
-        while left > 0:
-            k = min(self.S, left)
+        for subs in _passes(pattern, n_repeat, self.S):
             self.handle.barrier(channel=0)          # every rank's previous pass is complete
             s.launch_pass(self._peer_planes(s.nb.up, s.cur), self._peer_planes(s.nb.down, s.cur),
-                          coeffs, k)
+                          subs)
             s.flip()                                # all ranks flip in step: same parity everywhere
-            left -= k
         self.handle.barrier(channel=0)
+
+    def evolve(self, coeffs, n_steps):
+        self.run([tuple(coeffs)], n_steps)
+
+    def evolve_u4(self, theta, n_steps):
+        self.run(u4_pattern(theta), n_steps)
 
     def norm(self) -> float:
         return self.comm.all_reduce_sum(self.slab.norm_local())

@@ -110,6 +110,44 @@ def test_fused_peer_halo_path_matches_undivided_oracle(world, boundary, dtype):
     g.destroy()
 
 
+@pytest.mark.parametrize("world", [1, 3])
+@pytest.mark.parametrize("boundary", ["closed", "periodic"])
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("what", ["u4", "sep"])
+def test_fused_peer_halo_path_u4_and_separable_potential(world, boundary, dtype, what):
+    import torch
+    from paper_1208_2407_b200 import slab
+    dev = torch.device("cuda:0")
+    nx, ny = 252, 96
+    re, im, _ = G.random_inputs(nx, ny, dtype, 700 + world, False)
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    npdt = np.float32 if dtype == "f32" else np.float64
+    g = slab.PeerGroup(nx, ny, tdt, boundary, world, dev)
+    wre, wim = re.astype(np.float64), im.astype(np.float64)
+    d_re, d_im = torch.from_numpy(re).to(dev), torch.from_numpy(im).to(dev)
+    if what == "u4":
+        g.scatter(d_re, d_im)
+        g.evolve_u4(0.3, 4)                 # 20 sub-steps in passes of 6 (fp32) / 4 (fp64)
+        oracle.evolve_u4(wre, wim, 0.3, periodic=boundary == "periodic", n_steps=4)
+        scale = 4
+    else:
+        rng = np.random.default_rng(5)
+        Vx, Vy = rng.uniform(-6, 6, nx), rng.uniform(-6, 6, ny)
+        px = np.stack([np.cos(Vx), -np.sin(Vx)]).astype(npdt)
+        py = np.stack([np.cos(Vy), -np.sin(Vy)]).astype(npdt)
+        g.scatter(d_re, d_im, torch.from_numpy(px).to(dev), torch.from_numpy(py).to(dev))
+        g.evolve(coeffs(0.3), 11)
+        oracle.evolve_sep(wre, wim, *coeffs(0.3), px.astype(np.float64), py.astype(np.float64),
+                          periodic=boundary == "periodic", n_steps=11)
+        scale = 2
+    out_re = torch.empty((ny, nx), dtype=tdt, device=dev); out_im = torch.empty_like(out_re)
+    g.gather(out_re, out_im)
+    torch.cuda.synchronize()
+    err = max(np.abs(out_re.cpu().numpy() - wre).max(), np.abs(out_im.cpu().numpy() - wim).max())
+    assert err <= TIGHT[dtype] * scale, err
+    g.destroy()
+
+
 def test_slab_pass_argument_errors():
     import torch
     from paper_1208_2407_b200.binding import Plan, TsError
@@ -120,14 +158,14 @@ def test_slab_pass_argument_errors():
     short = (torch.zeros((4, 128), device=dev), torch.zeros((4, 128), device=dev))
     c = coeffs(0.1)
     with pytest.raises(TsError):
-        plan.slab_pass(a, a, None, None, *c, 2)              # in place
+        plan.slab_pass(a, a, None, None, [c] * 2)            # in place
     with pytest.raises(TsError):
-        plan.slab_pass(a, b, short, None, *c, 3)             # neighbour shorter than the halo
+        plan.slab_pass(a, b, short, None, [c] * 3)           # neighbour shorter than the halo
     with pytest.raises(TsError):
-        plan.slab_pass(a, b, None, None, *c, 7)              # deeper than the kernel goes
-    plan.slab_pass(a, b, short, short, *c, 2)
+        plan.slab_pass(a, b, None, None, [c] * 7)            # deeper than the kernel goes
+    plan.slab_pass(a, b, short, short, [c] * 2)
     plan.destroy()
     per = Plan(128, 16, torch.float32, "periodic")
     with pytest.raises(TsError):
-        per.slab_pass(a, b, None, None, *c, 1)               # slab plans are closed in y
+        per.slab_pass(a, b, None, None, [c])                 # slab plans are closed in y
     per.destroy()
