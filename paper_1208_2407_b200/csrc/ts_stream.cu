@@ -158,7 +158,9 @@ __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const Str
     ypair(a0, a1, p.te[J]);
     // closed lattice: the vertical-odd pair (yj-1, yj) does not exist at yj = 0 and yj = ny; the
     // ghost row is zero and stays zero (coupling 0), the real row takes 1/a per omitted sweep
-    const bool yedge = XEDGE && ((yj == 0 && p.edge_top) || (yj == p.ny && p.edge_bot));
+    constexpr bool SLAB = BND >= 3;      // row 0 / ny-1 may be a cut with a neighbour behind it
+    const bool yedge = XEDGE && ((yj == 0 && (!SLAB || p.edge_top)) ||
+                                 (yj == p.ny && (!SLAB || p.edge_bot)));
     const T t_yo = yedge ? T(0) : th;
     ypair(h, a0, t_yo);
     {
@@ -222,7 +224,9 @@ __device__ __forceinline__ void stream_stage_nopot(const StreamParams<T>& p,
     ypair(a0, a1, p.te[J]);
     // closed lattice: the vertical-odd pair (yj-1, yj) does not exist at yj = 0 and yj = ny; the
     // real row of the two takes 1/a instead (the ghost row is zero and stays zero)
-    const bool yedge = XEDGE && ((yj == 0 && p.edge_top) || (yj == p.ny && p.edge_bot));
+    constexpr bool SLAB = BND >= 3;      // row 0 / ny-1 may be a cut with a neighbour behind it
+    const bool yedge = XEDGE && ((yj == 0 && (!SLAB || p.edge_top)) ||
+                                 (yj == p.ny && (!SLAB || p.edge_bot)));
     const T t_yo = yedge ? T(0) : p.to[J];
     ypair(h, a0, t_yo);
     if (XEDGE) { const T sy = yedge ? p.sec_o[J] : T(1); scale_row(h, sy); scale_row(a0, sy); }
@@ -264,8 +268,11 @@ __global__ void __launch_bounds__(kWarps * 32, MINB)
 stream_kernel(const StreamParams<T> p) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     // BND: 0 = closed on both axes, 1 = periodic on both, 2 = periodic in x and closed in y (a row
-    // slab of a larger lattice, paper_1208_2407_b200/slab.py)
-    constexpr bool PERX = BND != 0, PERY = BND == 1;
+    // slab with stored halos, paper_1208_2407_b200/slab.py); 3 / 4 = closed / periodic in x, and in y
+    // a slab whose neighbours' rows are fetched in place (ts_slab_pass).  The peer logic is
+    // compiled in only there: as run-time branches it cost the closed kernels 13-18 %.
+    constexpr bool PERX = BND == 1 || BND == 2 || BND == 4, PERY = BND == 1, SLAB = BND >= 3;
+    const bool edge_top = !SLAB || p.edge_top, edge_bot = !SLAB || p.edge_bot;
     constexpr bool POT = PM == 1;             // phase planes travel through the ring
     constexpr int R = POT ? S + 1 : 1;        // iterations a ring slot stays live after its arrival
     constexpr uint32_t ROWB = kStripSites * sizeof(T);
@@ -341,17 +348,17 @@ stream_kernel(const StreamParams<T> p) {
 
     // fetch the next row pair into ring slot `slot` (one elected lane issues all copies)
     auto issue = [&](int slot) {
-        // where the row pair lives: own planes, or a neighbour's (slab with peer halos)
-        bool rowok = true;
+        // where the row pair lives: own planes -- or, beyond the slab, a neighbour's (ts_slab_pass)
+        bool rowok = PERY ? true : (fy >= 0 && fy < p.ny);
         const T* b_re = p.src_re;
         const T* b_im = p.src_im;
         int64_t off = foff;
-        if (!PERY) {
+        if (SLAB && !rowok) {
             if (fy < 0) {
                 rowok = p.up_re != nullptr && fy + p.up_rows >= 0;
                 b_re = p.up_re; b_im = p.up_im;
                 off = (int64_t)(fy + p.up_rows) * p.nx;
-            } else if (fy >= p.ny) {
+            } else {
                 rowok = p.dn_re != nullptr && fy - p.ny + 2 <= p.dn_rows;
                 b_re = p.dn_re; b_im = p.dn_im;
                 off = (int64_t)(fy - p.ny) * p.nx;
@@ -416,8 +423,8 @@ stream_kernel(const StreamParams<T> p) {
                 if (it + DIST < n_iter) issue(rs);
                 mbar_wait(bars + 8 * cs, cph);
                 const int y = y_in0 + 2 * it;
-                const bool rowok = !XEDGE || (c.xvalid && (y >= 0 || !p.edge_top) &&
-                                              (y < p.ny || !p.edge_bot));
+                const bool rowok = !XEDGE || (c.xvalid && (y >= 0 || !edge_top) &&
+                                              (y < p.ny || !edge_bot));
                 Row4<T> x0, x1;
                 if (rowok) {
                     const uint32_t base = c.ring + cs * SLOTB + c.lane_off;
@@ -445,8 +452,8 @@ stream_kernel(const StreamParams<T> p) {
         half(std::integral_constant<int, 1>{});
     }
     };   // run
-    const bool edge = c.xedge || (!PERY && ((y_in0 < 0 && p.edge_top) ||
-                                            (y_in0 + 2 * n_iter >= p.ny && p.edge_bot)));
+    const bool edge = c.xedge || (!PERY && ((y_in0 < 0 && edge_top) ||
+                                            (y_in0 + 2 * n_iter >= p.ny && edge_bot)));
     if (edge) run(std::true_type{});
     else run(std::false_type{});
 }
@@ -479,6 +486,10 @@ template <typename T, int S, int PM>
 int launch_b(const StreamParams<T>& p, int bnd, cudaStream_t st) {
     if (bnd == 1) return launch<T, S, PM, 1>(p, st);
     if (bnd == 2) return launch<T, S, PM, 2>(p, st);
+    if constexpr (PM != 1) {      // slabs with peer halos: no phase planes
+        if (bnd == 3) return launch<T, S, PM, 3>(p, st);
+        if (bnd == 4) return launch<T, S, PM, 4>(p, st);
+    }
     return launch<T, S, PM, 0>(p, st);
 }
 
@@ -571,7 +582,14 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
         if (j >= S) { p.to[j] = T(0); p.sec_o[j] = T(1); p.te[j + 1] = T(0); }
     }
     p.out_scale = (T)scale;
-    const int per = L.periodic_x ? (L.periodic_y ? 1 : 2) : 0;
+    int per = L.periodic_x ? (L.periodic_y ? 1 : 2) : 0;
+    if (peers) {
+        if (L.periodic_y || ph.mode == 1) {
+            set_error("stream_pass: peer halos need a closed-y plan and no phase planes");
+            return TS_EINVAL;
+        }
+        per = L.periodic_x ? 4 : 3;
+    }
     switch (S) {
         case 1: return launch_s<T, 1>(p, ph.mode, per, st);
         case 2: return launch_s<T, 2>(p, ph.mode, per, st);
