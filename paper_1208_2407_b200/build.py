@@ -13,7 +13,13 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 INCLUDE = PKG.parent / "include"
 LIB = PKG / "libts.so"
+# (source, object stem, extra flags); ts_stream.cu is compiled once per dtype so that its kernel
+# instantiations build in parallel
 SOURCES = ["ts_api.cu", "ts_generic.cu", "ts_fused.cu", "ts_stream.cu"]
+UNITS = [("ts_api.cu", "ts_api", []), ("ts_generic.cu", "ts_generic", []),
+         ("ts_fused.cu", "ts_fused", []),
+         ("ts_stream.cu", "ts_stream_f32", ["-DTS_STREAM_TU=32"]),
+         ("ts_stream.cu", "ts_stream_f64", ["-DTS_STREAM_TU=64"])]
 HEADERS = [CSRC / "ts_internal.h", CSRC / "ts_rows.cuh", INCLUDE / "ts.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]
@@ -43,9 +49,10 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         flags += ["-Xptxas", "-v"]
     objs = []
     procs = []
-    for s in SOURCES:
-        obj = CSRC / (s[:-3] + ".o")
-        cmd = [nvcc, *flags, "-I", str(INCLUDE), "-I", str(CSRC), "-c", str(CSRC / s), "-o", str(obj)]
+    for s, stem, extra in UNITS:
+        obj = CSRC / (stem + ".o")
+        cmd = [nvcc, *flags, *extra, "-I", str(INCLUDE), "-I", str(CSRC), "-c", str(CSRC / s),
+               "-o", str(obj)]
         procs.append((cmd, subprocess.Popen(cmd)))
         objs.append(str(obj))
     for cmd, p in procs:

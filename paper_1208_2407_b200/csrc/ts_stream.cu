@@ -609,6 +609,27 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
 
 }  // namespace
 
+// This file is compiled twice (build.py): once for fp32 (-DTS_STREAM_TU=32: defines
+// stream_pass_f32, the dispatcher and the defaults) and once for fp64 (-DTS_STREAM_TU=64: only
+// stream_pass_f64), so that the ~110 kernel instantiations build in parallel.
+#ifndef TS_STREAM_TU
+#define TS_STREAM_TU 0          // one translation unit with everything
+#endif
+
+#if TS_STREAM_TU == 0 || TS_STREAM_TU == 64
+int stream_pass_f64(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
+                    void* dst_im, const StepCoef* subs, const Phase& ph, int S, int seg_rows,
+                    int nst, cudaStream_t st, const Peers* peers) {
+    return pass_t<double>(L, (const double*)src_re, (const double*)src_im, (double*)dst_re,
+                          (double*)dst_im, subs, ph, S, seg_rows, nst, st, peers);
+}
+#endif
+
+#if TS_STREAM_TU == 0 || TS_STREAM_TU == 32
+int stream_pass_f64(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
+                    void* dst_im, const StepCoef* subs, const Phase& ph, int S, int seg_rows,
+                    int nst, cudaStream_t st, const Peers* peers);
+
 bool stream_supported(const LatticeDesc& L, const StepCoef& c) {
     // the strip window must split into at most two contiguous pieces of a row
     // (closed in x with periodic in y is not instantiated)
@@ -643,8 +664,9 @@ int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, vo
     if (L.dtype == TS_F32)
         return pass_t<float>(L, (const float*)src_re, (const float*)src_im, (float*)dst_re,
                              (float*)dst_im, subs, ph, S, seg_rows, nst, st, peers);
-    return pass_t<double>(L, (const double*)src_re, (const double*)src_im, (double*)dst_re,
-                          (double*)dst_im, subs, ph, S, seg_rows, nst, st, peers);
+    return stream_pass_f64(L, src_re, src_im, dst_re, dst_im, subs, ph, S, seg_rows, nst, st,
+                           peers);
 }
+#endif
 
 }  // namespace ts
