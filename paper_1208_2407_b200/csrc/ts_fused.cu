@@ -285,11 +285,11 @@ int fused_default_seg_rows(const LatticeDesc& L, int S, int blocks_per_sm) {
 int fused_default_steps(const LatticeDesc& L, bool pot) {
     // steps fused per pass, measured on B200 (profiles/r1d_probe.txt): fp32 without potential 6
     // (regrouped sweeps, packed FMAs; ts_evolve clamps to what the chosen kernel has) -- 4 on
-    // small lattices, where segments are short and the 2S warm-up iterations dominate; fp32 with
+    // small lattices (below 8 M sites), where segments are short and the 2S warm-up iterations dominate; fp32 with
     // potential 3; fp64 3 with, 4 without.
     if (L.dtype == TS_F32) {
         if (pot) return 3;
-        return L.nx * L.ny < (int64_t(1) << 22) ? 4 : 6;
+        return L.nx * L.ny < (int64_t(1) << 23) ? 4 : 6;
     }
     return pot ? 3 : 4;
 }

@@ -14,6 +14,7 @@
 // (double buffering); halo columns of a strip are recomputed and discarded
 // (PAPER.md:115).
 #include <math.h>
+#include <stdlib.h>
 
 #include <type_traits>
 
@@ -340,6 +341,14 @@ stream_kernel(const StreamParams<T> p) {
         mbar_fence_init();
     }
     __syncwarp();
+    // Programmatic dependent launch: the passes of one ts_evolve are launched with stream
+    // serialisation relaxed, so this grid's blocks may be scheduled (and get here) while the
+    // previous pass is still draining; nothing the previous pass wrote has been touched yet
+    // (px / the kernel parameters are inputs), and nothing is written before this point.
+    // griddepcontrol.wait returns once the previous grid has completed and its writes are visible;
+    // launch_dependents lets the next pass start its own prologue as early as possible.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;");
 
     // running row of the next fetch (warp-uniform): rows (fy, fy+1), element offset foff
     int fy = PERY ? wrap_index(y_in0, p.ny) : y_in0;
@@ -458,6 +467,15 @@ stream_kernel(const StreamParams<T> p) {
     else run(std::false_type{});
 }
 
+// programmatic dependent launch of consecutive passes (environment TS_NO_PDL=1 turns it off)
+bool stream_pdl() {
+    static const bool on = [] {
+        const char* e = getenv("TS_NO_PDL");
+        return !(e && e[0] == '1');
+    }();
+    return on;
+}
+
 template <typename T, int S, int PM, int BND>
 int launch(const StreamParams<T>& p, cudaStream_t st) {
     constexpr uint32_t SLOTB = (PM == 1 ? 8 : 4) * kStripSites * sizeof(T);
@@ -477,7 +495,25 @@ int launch(const StreamParams<T>& p, cudaStream_t st) {
     }
     const int n_seg = (p.ny + p.seg_rows - 1) / p.seg_rows;
     dim3 grid((p.n_strips + kWarps - 1) / kWarps, n_seg);
-    kern<<<grid, kWarps * 32, smem, st>>>(p);
+    // programmatic dependent launch pays where launch latency and the prologue are a visible part
+    // of a pass, i.e. for grids of at most one wave (1024^2 +12 %, 2048^2 +17 %, 4096^2 +0-2 %);
+    // on many-wave grids the next pass's blocks then start in lockstep and a 16384^2 pass gets
+    // ~8 % slower (probe r1f pdl/pdl2), so those keep the ordinary launch
+    if (stream_pdl() && (int64_t)grid.x * grid.y <= 148 * 3) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = grid;
+        cfg.blockDim = dim3(kWarps * 32);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        TS_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, p));
+    } else {
+        kern<<<grid, kWarps * 32, smem, st>>>(p);
+    }
     TS_CUDA_TRY(cudaGetLastError());
     return TS_OK;
 }
