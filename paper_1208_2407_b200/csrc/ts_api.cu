@@ -277,7 +277,7 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
     if (rc != TS_OK) return rc;
 
     if (plan->opt_variant == 2 && !can_stream)
-        return fail(TS_EUNSUPPORTED, "the TMA ring kernel needs nx >= 128");
+        return fail(TS_EUNSUPPORTED, "the TMA ring kernel needs nx >= 128 on a lattice that is periodic in x");
     if (plan->opt_variant == 1 && !can_v1)
         return fail(TS_EUNSUPPORTED, "the register-prefetch kernel needs one boundary type on both axes");
     const bool use_stream = can_stream && plan->opt_variant != 1;

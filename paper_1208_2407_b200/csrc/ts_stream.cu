@@ -669,7 +669,10 @@ int stream_pass_f64(const LatticeDesc& L, const void* src_re, const void* src_im
 bool stream_supported(const LatticeDesc& L, const StepCoef& c) {
     // the strip window must split into at most two contiguous pieces of a row
     // (closed in x with periodic in y is not instantiated)
-    return fused_shape_ok(L, c) && L.nx >= kStripSites && (L.periodic_x || !L.periodic_y);
+    // (periodic in x: the 128-wide window may wrap once, so the row must be at least that long;
+    // closed in x: any width, columns beyond the lattice are ghost lanes)
+    return fused_shape_ok(L, c) && (L.nx >= kStripSites || !L.periodic_x) &&
+           (L.periodic_x || !L.periodic_y);
 }
 
 int stream_max_steps(const LatticeDesc& L, bool pot) {

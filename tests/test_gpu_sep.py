@@ -63,7 +63,7 @@ def test_sep_stream_kernel(nx, ny, boundary, dtype, fuse):
         assert info["passes"] == math.ceil(9 / fuse)
 
 
-@pytest.mark.parametrize("nx,ny,opts", [(64, 64, dict(path=2, variant=1)), (124, 34, dict(path=2)),
+@pytest.mark.parametrize("nx,ny,opts", [(64, 64, dict(path=2, variant=1)), (124, 34, dict(path=2, variant=1)),
                                         (129, 67, dict()), (256, 30, dict(path=1))])
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 def test_sep_other_paths_write_the_product_out(nx, ny, opts, dtype):
