@@ -91,3 +91,16 @@ def test_slab_shorter_than_halo_is_rejected():
     with pytest.raises(ValueError):
         slab.LocalGroup(8, 16, torch.float64, "closed", 4, steps_per_exchange=4,
                         evolve_fn=oracle_evolve_fn, norm_fn=oracle_norm_fn)
+
+
+def test_pass_cutting_and_u4_pattern():
+    pat = slab.u4_pattern(0.3)
+    assert len(pat) == 5 and pat[0] == pat[1] == pat[3] == pat[4] != pat[2]
+    # the five angles sum to theta: cos/sin of the summed half angles
+    half = sum(math.atan2(c[1], c[0]) for c in pat)
+    assert abs(half - 0.15) < 1e-15
+    passes = list(slab._passes(pat, 4, 6))          # 20 sub-steps in passes of at most 6
+    assert [len(p) for p in passes] == [6, 6, 6, 2]
+    flat = [c for p in passes for c in p]
+    assert flat == pat * 4
+    assert list(slab._passes([slab.step_coeffs(0.1)], 0, 6)) == []
