@@ -119,6 +119,19 @@ int ts_evolve_sep(ts_plan* plan, void* psi_re, void* psi_im,
                   const void* phase_x, const void* phase_y, int64_t n_steps, void* cuda_stream);
 
 /*
+ * ts_evolve_tdep -- ts_evolve for a TIME-DEPENDENT potential (the Hamiltonian may
+ * depend on time): step k (k = 0 .. n_steps-1) uses the phase planes pot_phases[k].
+ *   pot_phases   HOST array of n_steps DEVICE pointers, each laid out like pot_phase of ts_evolve
+ *                (NULL entry = that step has no potential and is the 7-stage step).
+ * Steps are fused into one pass only while they share the same phase array, so a potential that
+ * changes every step costs one pass over HBM per step (24 B per site in fp32).  Other arguments,
+ * asynchrony (the pointer list is read before the call returns) and errors as for ts_evolve.
+ */
+int ts_evolve_tdep(ts_plan* plan, void* psi_re, void* psi_im,
+                   double a_half, double b_half, double a_full, double b_full,
+                   const void* const* pot_phases, int64_t n_steps, void* cuda_stream);
+
+/*
  * ts_slab_pass -- ONE fused pass over a row slab of a larger lattice, halos read in place from
  * the neighbouring slabs: dst <- U2(c[n_sub-1]) ... U2(c[0]) src on the plan's nx x ny rows, where
  * the rows above row 0 are the LAST up_rows rows of (up_re, up_im) and the rows below row ny-1

@@ -152,6 +152,14 @@ def evolve_sep(re, im, a_half, b_half, a_full, b_full, phase_x, phase_y, periodi
            n_steps=n_steps)
 
 
+def evolve_tdep(re, im, a_half, b_half, a_full, b_full, pots, periodic=False) -> None:
+    """In place: one second-order step per entry of `pots`, step k with the potential phase
+    pots[k] = (pot_re, pot_im) or None (time-dependent Hamiltonian): by definition
+    a chain of single steps of ``evolve``."""
+    for pot in pots:
+        evolve(re, im, a_half, b_half, a_full, b_full, pot=pot, periodic=periodic, n_steps=1)
+
+
 # p of Eq. 4 (PAPER.md:95-101): p = (4 - 4^(1/3))^-1
 U4_P = 1.0 / (4.0 - 4.0 ** (1.0 / 3.0))
 

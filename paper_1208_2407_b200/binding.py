@@ -13,7 +13,7 @@ TS_MAX_FUSE = 6
 _LIB_PATH = Path(__file__).resolve().parent / "libts.so"
 _lib = None
 
-SYMBOLS = ["ts_plan_create", "ts_plan_create_xy", "ts_evolve", "ts_evolve_u4", "ts_evolve_sep", "ts_slab_pass",
+SYMBOLS = ["ts_plan_create", "ts_plan_create_xy", "ts_evolve", "ts_evolve_u4", "ts_evolve_sep", "ts_evolve_tdep", "ts_slab_pass",
            "ts_norm", "ts_evolve_host", "ts_plan_set_option",
            "ts_plan_get_info", "ts_plan_destroy", "ts_last_error"]
 
@@ -43,6 +43,8 @@ def lib():
         L.ts_evolve_u4.restype = i32
         L.ts_evolve_sep.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp, vp, i64, vp]
         L.ts_evolve_sep.restype = i32
+        L.ts_evolve_tdep.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, ctypes.POINTER(vp), i64, vp]
+        L.ts_evolve_tdep.restype = i32
         L.ts_slab_pass.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, vp, vp, i64,
                                    ctypes.POINTER(dbl), i32, vp, vp, i64, i64, i32, vp]
         L.ts_slab_pass.restype = i32
@@ -154,6 +156,18 @@ class Plan:
                                   ctypes.c_void_p(psi_im.data_ptr()), float(theta),
                                   self._pot_ptr(pot_phase_p), self._pot_ptr(pot_phase_q),
                                   int(n_steps), _stream_handle(stream)))
+
+    def evolve_tdep(self, psi_re, psi_im, a_half, b_half, a_full, b_full, pot_phases, stream=None):
+        """ts_evolve_tdep: one step per entry of pot_phases (CUDA tensors [2][ny][nx] or None)."""
+        self._planes(psi_re, psi_im)
+        n = len(pot_phases)
+        arr = (ctypes.c_void_p * max(n, 1))()
+        for k, t in enumerate(pot_phases):
+            p = self._pot_ptr(t)
+            arr[k] = p.value if p is not None else None
+        _check(lib().ts_evolve_tdep(self._h, ctypes.c_void_p(psi_re.data_ptr()),
+                                    ctypes.c_void_p(psi_im.data_ptr()), a_half, b_half, a_full,
+                                    b_full, arr, n, _stream_handle(stream)))
 
     def evolve_sep(self, psi_re, psi_im, a_half, b_half, a_full, b_full, phase_x, phase_y,
                    n_steps=1, stream=None):

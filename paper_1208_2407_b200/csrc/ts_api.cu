@@ -416,6 +416,27 @@ int ts_slab_pass(ts_plan* plan, const void* src_re, const void* src_im, void* ds
     return TS_OK;
 }
 
+int ts_evolve_tdep(ts_plan* plan, void* psi_re, void* psi_im, double a_half, double b_half,
+                   double a_full, double b_full, const void* const* pot_phases, int64_t n_steps,
+                   void* cuda_stream) {
+    if (n_steps < 0) return fail(TS_EINVAL, "n_steps < 0");
+    if (n_steps > 0 && !pot_phases) return fail(TS_EINVAL, "NULL list of potential phases");
+    if (n_steps > (int64_t(1) << 24)) return fail(TS_EINVAL, "n_steps too large for one call");
+    // one sub-step per time step, each with its own phase array: consecutive steps that happen to
+    // share an array are still fused into one pass
+    SubStep* pat = n_steps ? new (std::nothrow) SubStep[(size_t)n_steps] : nullptr;
+    if (n_steps && !pat) return fail(TS_EALLOC, "out of host memory");
+    for (int64_t k = 0; k < n_steps; ++k) {
+        pat[k].c = ts::StepCoef{a_half, b_half, a_full, b_full};
+        pat[k].ph = ts::Phase{pot_phases[k] ? 1 : 0, pot_phases[k], nullptr, nullptr};
+    }
+    const SubStep none{{a_half, b_half, a_full, b_full}, ts::Phase{0, nullptr, nullptr, nullptr}};
+    const int rc = n_steps ? evolve_pattern(plan, psi_re, psi_im, pat, (int)n_steps, 1, cuda_stream)
+                           : evolve_pattern(plan, psi_re, psi_im, &none, 1, 0, cuda_stream);
+    delete[] pat;
+    return rc;
+}
+
 int ts_evolve_u4(ts_plan* plan, void* psi_re, void* psi_im, double theta, const void* pot_p,
                  const void* pot_q, int64_t n_steps, void* cuda_stream) {
     if ((pot_p == nullptr) != (pot_q == nullptr))

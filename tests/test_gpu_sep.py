@@ -69,3 +69,43 @@ def test_sep_stream_kernel(nx, ny, boundary, dtype, fuse):
 def test_sep_other_paths_write_the_product_out(nx, ny, opts, dtype):
     info = run(nx, ny, dtype, "closed", 5, nx + ny, **opts)
     assert info["variant"] != 2
+
+
+@pytest.mark.parametrize("nx,ny,opts", [(252, 66, dict(path=2, variant=2)), (64, 64, dict()),
+                                        (129, 67, dict())])
+@pytest.mark.parametrize("boundary", ["closed", "periodic"])
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_time_dependent_potential(nx, ny, opts, boundary, dtype):
+    # ts_evolve_tdep: a new phase array per step, with a repeated array (fused into one pass) and a
+    # step without potential in between
+    import torch
+    from paper_1208_2407_b200.binding import Plan
+    if boundary == "periodic" and (nx % 2 or ny % 2):
+        pytest.skip("periodic needs even sizes")
+    dev = torch.device("cuda:0")
+    re, im, _ = G.random_inputs(nx, ny, dtype, nx + ny, False)
+    rng = np.random.default_rng(11)
+    npdt = np.float32 if dtype == "f32" else np.float64
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    arrays = []
+    for _ in range(3):
+        V = rng.uniform(-5, 5, (ny, nx))
+        arrays.append(np.stack([np.cos(V), -np.sin(V)]).astype(npdt))
+    order = [0, 1, 1, None, 2, 0, 0, 0]
+    dpots = [torch.from_numpy(a).to(dev) for a in arrays]
+    plan = Plan(nx, ny, tdt, boundary)
+    for k, v in opts.items():
+        plan.set_option(k, v)
+    dre, dim = torch.from_numpy(re).to(dev), torch.from_numpy(im).to(dev)
+    plan.evolve_tdep(dre, dim, *coeffs(0.3), [None if k is None else dpots[k] for k in order])
+    torch.cuda.synchronize()
+    wre, wim = re.astype(np.float64), im.astype(np.float64)
+    opots = [None if k is None else (arrays[k][0].astype(np.float64), arrays[k][1].astype(np.float64))
+             for k in order]
+    oracle.evolve_tdep(wre, wim, *coeffs(0.3), opots, periodic=boundary == "periodic")
+    err = max(np.abs(dre.cpu().numpy() - wre).max(), np.abs(dim.cpu().numpy() - wim).max())
+    assert err <= TIGHT[dtype] * 2, err
+    if opts.get("variant") == 2:
+        assert plan.info("passes") == 5          # runs: 0 | 1 1 | none | 2 | 0 0 0
+    plan.evolve_tdep(dre, dim, *coeffs(0.3), [])   # no steps: a no-op
+    plan.destroy()
