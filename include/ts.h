@@ -184,13 +184,19 @@ int ts_evolve_host(ts_plan* plan, void* psi_re_host, void* psi_im_host,
  * ts_plan_set_option -- tuning knobs, all optional.  Unknown names give TS_EINVAL.
  *   "path"         0 = auto, 1 = generic per-sweep kernels only, 2 = fused kernel required
  *                  (ts_evolve then returns TS_EUNSUPPORTED for shapes the fused kernel cannot take).
- *   "fuse_steps"   steps fused per pass over HBM (1..TS_MAX_FUSE), 0 = auto.
- *   "seg_rows"     rows of output per streaming segment of the fused kernel, 0 = auto.
+ *   "fuse_steps"   steps fused per pass over HBM (1..TS_MAX_FUSE; 5 and 6 only fp32 without phase
+ *                  planes on the TMA ring kernel), 0 = auto.
+ *   "seg_rows"     rows of output per streaming segment of the fused kernel (even), 0 = auto.
+ *   "variant"      0 = auto, 1 = register-prefetch kernel, 2 = TMA ring kernel (the default
+ *                  wherever it applies: nx >= 128 or closed in x).
+ *   "ring_slots"   row-pair slots of the TMA ring per warp, 0 = auto.
+ * Environment: TS_NO_PDL=1 turns off programmatic dependent launch between passes.
  */
 int ts_plan_set_option(ts_plan* plan, const char* name, int64_t value);
 
-/* ts_plan_get_info -- read back what the last ts_evolve used:
- *   "fused" (0/1), "fuse_steps", "passes", "launches" (kernels + copies enqueued), "seg_rows". */
+/* ts_plan_get_info -- read back what the last ts_evolve* / ts_slab_pass used:
+ *   "fused" (0/1), "fuse_steps", "passes", "launches" (kernels + copies enqueued), "seg_rows",
+ *   "variant" (1 / 2, 0 on the per-sweep path). */
 int ts_plan_get_info(const ts_plan* plan, const char* name, int64_t* out_value);
 
 int ts_plan_destroy(ts_plan* plan);           /* NULL is accepted (no-op, TS_OK) */
