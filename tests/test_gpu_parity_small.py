@@ -118,6 +118,23 @@ def test_full_angle_coefficients_need_not_be_twice_the_half_angle(boundary, fuse
     assert err < 2e-5, (err, info)
 
 
+@pytest.mark.parametrize("theta,expect_fused", [(0.0, 1), (-0.7, 1), (1.2, 1), (1.4, 0), (2.9, 0)])
+@pytest.mark.parametrize("with_pot", [False, True])
+def test_angle_range(theta, expect_fused, with_pot):
+    # the fused kernels use tangents: they take angles with cos(theta) > 0.25 (theta = 0: the
+    # identity, negative: backwards in time); beyond that the automatic path is the per-sweep one
+    nx, ny, n = 252, 66, 5
+    cfg = G.make_cfg(nx, ny, "f64", "closed", theta, n)
+    re, im, pot = G.random_inputs(nx, ny, "f64", 17, with_pot)
+    got_re, got_im, info = G.gpu_evolve(cfg, re, im, pot, n_steps=n)
+    want_re, want_im = G.oracle_evolve(cfg, re, im, pot, n_steps=n)
+    err, _ = G.errors(cfg, got_re, got_im, want_re, want_im)
+    assert info["fused"] == expect_fused, info
+    assert err < 1e-12, (err, info)
+    if theta == 0.0 and not with_pot:
+        assert np.abs(got_re - re).max() < 1e-15 and np.abs(got_im - im).max() < 1e-15
+
+
 def test_auto_path_picks_generic_for_unaligned_shapes():
     cfg = G.make_cfg(130, 31, "f32", "closed", 0.2, 4)
     re, im, pot = G.random_inputs(130, 31, "f32", 5, True)
