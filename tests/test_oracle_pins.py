@@ -329,3 +329,62 @@ def test_evolve_sep_is_evolve_with_the_sum_potential():
     oracle.evolve_sep(r2, i2, *coeffs(theta), (np.cos(Vx), -np.sin(Vx)), (np.cos(Vy), -np.sin(Vy)),
                       periodic=True, n_steps=4)
     assert np.abs(re - r2).max() < 1e-14 and np.abs(im - i2).max() < 1e-14
+
+
+# --- physics of the whole step: group velocity of a wavepacket (tight-binding dispersion) ---------
+def test_wavepacket_moves_with_the_tight_binding_group_velocity():
+    # H = -J * Adj has E(k) = -2J (cos kx + cos ky), so a packet of mean momentum k drifts by
+    # dE/dk = 2J sin k per unit time: per step of angle theta = J dt that is 2 theta sin k sites.
+    # Checks sign (R1: +i b, so positive k moves to +x), the half-angle reading (R2: a step is ONE
+    # dt, not two) and the x/y assignment, independently of any matrix code.
+    nx = ny = 96
+    kx, ky, sigma, theta, n = 0.5, -0.3, 8.0, 0.05, 60
+    x = np.arange(nx)[None, :] - 40.0
+    y = np.arange(ny)[:, None] - 52.0
+    env = np.exp(-(x * x + y * y) / (4 * sigma * sigma))
+    re = env * np.cos(kx * x + ky * y)
+    im = env * np.sin(kx * x + ky * y)
+    nrm = math.sqrt((re * re + im * im).sum())
+    re, im = np.ascontiguousarray(re / nrm), np.ascontiguousarray(im / nrm)
+
+    def centre(r, i):
+        p = r * r + i * i
+        return (p * np.arange(nx)[None, :]).sum(), (p * np.arange(ny)[:, None]).sum()
+
+    x0, y0 = centre(re, im)
+    oracle.evolve(re, im, *coeffs(theta), periodic=False, n_steps=n)
+    x1, y1 = centre(re, im)
+    # finite width in k: <sin k> = sin(k0) exp(-1/(8 sigma^2)) for a Gaussian of std 1/(2 sigma)
+    damp = math.exp(-1.0 / (8 * sigma * sigma))
+    want_dx = 2 * theta * n * math.sin(kx) * damp
+    want_dy = 2 * theta * n * math.sin(ky) * damp
+    assert abs((x1 - x0) - want_dx) < 0.02 * abs(want_dx), (x1 - x0, want_dx)
+    assert abs((y1 - y0) - want_dy) < 0.02 * abs(want_dy), (y1 - y0, want_dy)
+
+
+def test_packet_in_a_harmonic_trap_oscillates_at_the_classical_frequency():
+    # small momenta: E(k) ~ -2J + J k^2, an effective mass m = 1/(2J); in V = w^2 x^2 / 2 the
+    # packet centre follows x_c + A cos(W t), W = w sqrt(2J) (Ehrenfest).  Pins the SIGN of the
+    # potential phase (R9: exp(-i V dt); with +i the trap repels) and its place in the step.
+    nx, ny = 192, 4
+    J, w, A, dt = 0.25, 0.02, 12.0, 1.0
+    W = w * math.sqrt(2 * J)
+    sigma = math.sqrt(J / W) / math.sqrt(2) * math.sqrt(2)      # ground-state width of |psi|^2
+    xc = 96.0
+    x = np.arange(nx)[None, :] - xc
+    env = np.exp(-((x - A) ** 2) / (4 * sigma * sigma)) * np.ones((ny, 1))
+    re = np.ascontiguousarray(env / math.sqrt((env * env).sum()))
+    im = np.zeros_like(re)
+    V = 0.5 * w * w * (x * x) * np.ones((ny, 1))
+    pot = (np.cos(V * dt), -np.sin(V * dt))
+    quarter = int(round(math.pi / (2 * W)))
+
+    def centre(r, i):
+        p = r * r + i * i
+        return (p * np.arange(nx)[None, :]).sum() / p.sum() - xc
+
+    assert abs(centre(re, im) - A) < 1e-9
+    oracle.evolve(re, im, *coeffs(J * dt), pot=pot, periodic=True, n_steps=quarter)
+    assert abs(centre(re, im)) < 0.06 * A, centre(re, im)            # through the centre
+    oracle.evolve(re, im, *coeffs(J * dt), pot=pot, periodic=True, n_steps=quarter)
+    assert abs(centre(re, im) + A) < 0.06 * A, centre(re, im)        # at the other turning point
