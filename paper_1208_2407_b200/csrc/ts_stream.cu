@@ -16,6 +16,7 @@
 #include <math.h>
 #include <stdlib.h>
 
+#include <atomic>
 #include <type_traits>
 
 #include "ts_internal.h"
@@ -27,6 +28,7 @@ namespace {
 using namespace rows;
 
 constexpr int kWarps = 4;
+constexpr int kMaxDevices = 64;
 
 
 template <typename T>
@@ -487,11 +489,16 @@ int launch(const StreamParams<T>& p, cudaStream_t st) {
 #endif
     constexpr int MINB = sizeof(T) == 4 ? TS_MINB_F32 : (S <= 2 ? 3 : 2);
     auto kern = stream_kernel<T, S, PM, BND, MINB>;
-    static size_t configured = 0;    // per instantiation
-    if (smem > configured) {
+    // the opt-in for > 48 KB of dynamic shared memory is a per-device, per-kernel attribute:
+    // remembered per instantiation and device (atomics: plans on different threads may race here,
+    // setting it twice is harmless)
+    static std::atomic<size_t> configured[kMaxDevices];
+    int dev = 0;
+    TS_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices || smem > configured[dev].load(std::memory_order_relaxed)) {
         TS_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)smem));
-        configured = smem;
+        if (dev >= 0 && dev < kMaxDevices) configured[dev].store(smem, std::memory_order_relaxed);
     }
     const int n_seg = (p.ny + p.seg_rows - 1) / p.seg_rows;
     dim3 grid((p.n_strips + kWarps - 1) / kWarps, n_seg);
