@@ -188,7 +188,10 @@ int ts_evolve_host(ts_plan* plan, void* psi_re_host, void* psi_im_host,
  *                  planes on the TMA ring kernel), 0 = auto.
  *   "seg_rows"     rows of output per streaming segment of the fused kernel (even), 0 = auto.
  *   "variant"      0 = auto, 1 = register-prefetch kernel, 2 = TMA ring kernel (the default
- *                  wherever it applies: nx >= 128 or closed in x).
+ *                  wherever it applies: nx >= 128 or closed in x), 3 = on-chip-resident kernel:
+ *                  the whole lattice in the registers of one thread block and all n_steps in
+ *                  one launch (the default for uniform steps on lattices up to 128 x 128 sites in
+ *                  fp32, 128 x 64 in fp64, half that with a potential).
  *   "ring_slots"   row-pair slots of the TMA ring per warp, 0 = auto.
  * Environment: TS_NO_PDL=1 turns off programmatic dependent launch between passes.
  */
@@ -196,7 +199,7 @@ int ts_plan_set_option(ts_plan* plan, const char* name, int64_t value);
 
 /* ts_plan_get_info -- read back what the last ts_evolve* / ts_slab_pass used:
  *   "fused" (0/1), "fuse_steps", "passes", "launches" (kernels + copies enqueued), "seg_rows",
- *   "variant" (1 / 2, 0 on the per-sweep path). */
+ *   "variant" (1 / 2 / 3, 0 on the per-sweep path). */
 int ts_plan_get_info(const ts_plan* plan, const char* name, int64_t* out_value);
 
 int ts_plan_destroy(ts_plan* plan);           /* NULL is accepted (no-op, TS_OK) */

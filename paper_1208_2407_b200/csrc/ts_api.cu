@@ -145,7 +145,7 @@ int ts_plan_set_option(ts_plan* plan, const char* name, int64_t value) {
         if (value < 0 || value % 2) return fail(TS_EINVAL, "seg_rows must be even and >= 0");
         plan->opt_seg = value;
     } else if (!strcmp(name, "variant")) {
-        if (value < 0 || value > 2) return fail(TS_EINVAL, "variant must be 0, 1 or 2");
+        if (value < 0 || value > 3) return fail(TS_EINVAL, "variant must be 0, 1, 2 or 3");
         plan->opt_variant = value;
     } else if (!strcmp(name, "ring_slots")) {
         if (value < 0 || value > 64) return fail(TS_EINVAL, "ring_slots out of range");
@@ -235,6 +235,20 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
     if (period > 1 && n_repeat > (int64_t(1) << 56)) return fail(TS_EINVAL, "n_steps too large");
     const int64_t n_sub = n_repeat * period;
 
+    // tiny lattices: the whole evolution in one launch of the on-chip-resident kernel (uniform
+    // steps, no or plane potential)
+    const bool can_tiny = period == 1 && pat[0].ph.mode != 2 &&
+                          ts::tiny_supported(L, pat[0].c, pat[0].ph.mode == 1);
+    if (plan->opt_variant == 3 && !can_tiny)
+        return fail(TS_EUNSUPPORTED, "the on-chip kernel takes uniform steps on lattices of at most "
+                                     "128 x 128 (fp32) / 128 x 64 (fp64) sites, half with a potential");
+    if (can_tiny && plan->opt_path != 1 && (plan->opt_variant == 0 || plan->opt_variant == 3)) {
+        rc = ts::tiny_evolve(L, psi_re, psi_im, pat[0].c, pat[0].ph.planes, n_repeat, st);
+        if (rc != TS_OK) return rc;
+        plan->info_fused = 1; plan->info_fuse = n_repeat; plan->info_passes = 1;
+        plan->info_launches = 1; plan->info_seg = L.ny; plan->info_variant = 3;
+        return TS_OK;
+    }
     if (plan->opt_path == 2 && !can_fuse)
         return fail(TS_EUNSUPPORTED,
                     "fused kernel needs nx % 4 == 0, even ny and cos(theta) > 0.25");
