@@ -186,7 +186,8 @@ int ts_evolve_host(ts_plan* plan, void* psi_re_host, void* psi_im_host,
  *                  (ts_evolve then returns TS_EUNSUPPORTED for shapes the fused kernel cannot take).
  *   "fuse_steps"   steps fused per pass over HBM (1..TS_MAX_FUSE; 5 and 6 only fp32 without phase
  *                  planes on the TMA ring kernel), 0 = auto.
- *   "seg_rows"     rows of output per streaming segment of the fused kernel (even), 0 = auto.
+ *   "seg_rows"     rows of output per streaming segment of the fused kernel (even), 0 = auto;
+ *                  for the on-chip kernel (variant 3): rows per warp, 2 / 4 / 8, 0 = auto.
  *   "variant"      0 = auto, 1 = register-prefetch kernel, 2 = TMA ring kernel (the default
  *                  wherever it applies: nx >= 128 or closed in x), 3 = on-chip-resident kernel:
  *                  the whole lattice in the registers of one thread block and all n_steps in

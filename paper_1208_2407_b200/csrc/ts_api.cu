@@ -243,7 +243,8 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
         return fail(TS_EUNSUPPORTED, "the on-chip kernel takes uniform steps on lattices of at most "
                                      "128 x 128 (fp32) / 128 x 64 (fp64) sites, half with a potential");
     if (can_tiny && plan->opt_path != 1 && (plan->opt_variant == 0 || plan->opt_variant == 3)) {
-        rc = ts::tiny_evolve(L, psi_re, psi_im, pat[0].c, pat[0].ph.planes, n_repeat, st);
+        rc = ts::tiny_evolve(L, psi_re, psi_im, pat[0].c, pat[0].ph.planes, n_repeat,
+                             (int)plan->opt_seg, st);     // "seg_rows" = rows per warp here
         if (rc != TS_OK) return rc;
         plan->info_fused = 1; plan->info_fuse = n_repeat; plan->info_passes = 1;
         plan->info_launches = 1; plan->info_seg = L.ny; plan->info_variant = 3;

@@ -72,10 +72,10 @@ int fused_pass(const LatticeDesc& L, const void* src_re, const void* src_im, voi
 int fused_default_seg_rows(const LatticeDesc& L, int S, int blocks_per_sm = 3);
 
 // ---- on-chip-resident path for tiny lattices (ts_tiny.cu): the whole evolution in one launch -----
-int tiny_rows_per_warp(const LatticeDesc& L, bool pot);
+int tiny_rows_per_warp(const LatticeDesc& L, bool pot, int prefer);   // prefer 4: 4 rows if possible
 bool tiny_supported(const LatticeDesc& L, const StepCoef& c, bool pot);
 int tiny_evolve(const LatticeDesc& L, void* re, void* im, const StepCoef& c, const void* pot,
-                int64_t n_steps, cudaStream_t st);
+                int64_t n_steps, int rows_per_warp, cudaStream_t st);
 
 // ---- fused streaming path v2 (ts_stream.cu): TMA bulk copies into a per-warp smem ring ---------
 bool stream_supported(const LatticeDesc& L, const StepCoef& c);

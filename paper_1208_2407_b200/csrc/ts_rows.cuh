@@ -191,6 +191,15 @@ __device__ __forceinline__ void scale_row(Row4<T>& r, T s) {
 #pragma unroll
     for (int i = 0; i < 4; ++i) { r.re[i] *= s; r.im[i] *= s; }
 }
+#ifndef TS_SCALAR_F32
+__device__ __forceinline__ void scale_row(Row4<float>& r, float s) {
+#pragma unroll
+    for (int k = 0; k < 4; k += 2) {
+        mul2v(r.re[k], r.re[k + 1], r.re[k], r.re[k + 1], s, s);
+        mul2v(r.im[k], r.im[k + 1], r.im[k], r.im[k + 1], s, s);
+    }
+}
+#endif
 
 // psi <- psi * (pr + i pi) on one row
 template <typename T>

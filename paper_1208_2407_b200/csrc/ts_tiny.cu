@@ -31,8 +31,9 @@ struct TinyParams {
     int nx, ny;
     int64_t n_steps;
     T t_h, t_f, sec_h, sec_f;
-    T step_scale;     // a_h^6 a_f without potential, a_h^8 with, rounded to T
-    T final_scale;    // (exact / rounded step scale)^n_steps: undoes the accumulated rounding
+    T scale4;         // deferred cosines of FOUR steps, (a_h^6 a_f)^4 or a_h^32, rounded to T
+    T final_scale;    // the steps after the last multiple of four, and the accumulated rounding
+                      // of scale4 taken out again
 };
 
 // me <- me + i t other (one side of a pair rotation whose partner lives in another warp)
@@ -79,11 +80,11 @@ __device__ __forceinline__ void xo_ring(Row4<T>& r, T t, int up_src, int dn_src)
 }
 
 // threads per block the register budget allows: fp32 rows cost 8 registers each, fp64 16
-template <typename T>
-constexpr int tiny_max_threads() { return sizeof(T) == 4 ? 1024 : 512; }
+template <typename T, int R>
+constexpr int tiny_max_threads() { return R >= 8 ? 256 : (sizeof(T) == 4 ? 1024 : 512); }
 
 template <typename T, int R, bool POT, bool PER>
-__global__ void __launch_bounds__(tiny_max_threads<T>(), 1) tiny_kernel(const TinyParams<T> p) {
+__global__ void __launch_bounds__(tiny_max_threads<T, R>(), 1) tiny_kernel(const TinyParams<T> p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     // per warp: its top row and its bottom row, [warp][top|bottom][re|im][lane][4]
     T* xch = reinterpret_cast<T*>(smem_raw);
@@ -186,8 +187,10 @@ __global__ void __launch_bounds__(tiny_max_threads<T>(), 1) tiny_kernel(const Ti
         y_even(p.t_h);
         x_odd();
         x_even(p.t_h);
+        if ((s & 3) == 3) {     // every fourth step: keeps the scaled amplitudes in range
 #pragma unroll
-        for (int i = 0; i < R; ++i) scale_row(row[i], p.step_scale);
+            for (int i = 0; i < R; ++i) scale_row(row[i], p.scale4);
+        }
     }
 
     if (active) {
@@ -220,8 +223,8 @@ int launch_r(const TinyParams<T>& p, bool pot, bool per, int nw, cudaStream_t st
 
 template <typename T>
 int evolve_t(const LatticeDesc& L, T* re, T* im, const StepCoef& c, const T* pot, int64_t n_steps,
-             cudaStream_t st) {
-    const int R = tiny_rows_per_warp(L, pot != nullptr);
+             int prefer, cudaStream_t st) {
+    const int R = tiny_rows_per_warp(L, pot != nullptr, prefer);
     TinyParams<T> p;
     p.re = re; p.im = im;
     p.pot_re = pot; p.pot_im = pot ? pot + L.nx * L.ny : nullptr;
@@ -229,42 +232,59 @@ int evolve_t(const LatticeDesc& L, T* re, T* im, const StepCoef& c, const T* pot
     p.t_h = (T)(c.b_h / c.a_h); p.t_f = (T)(c.b_f / c.a_f);
     p.sec_h = (T)(1.0 / c.a_h); p.sec_f = (T)(1.0 / c.a_f);
     const double step = pot ? pow(c.a_h, 8) : pow(c.a_h, 6) * c.a_f;
-    p.step_scale = (T)step;
-    // the rounded factor is applied n_steps times: its relative error would add up linearly
-    // (fp32: 6e-8 per step, 2e-4 in the norm after 1000 steps); the store takes it out again
-    p.final_scale = (T)exp((double)n_steps * log(step / (double)p.step_scale));
+    p.scale4 = (T)pow(step, 4);
+    // the rounded factor is applied n_steps / 4 times: its relative error would add up linearly
+    // (2e-4 in the fp32 norm after 1000 steps when applied per step); the store takes it out
+    // again, together with the cosines of the last n_steps % 4 steps
+    const int64_t groups = n_steps / 4;
+    p.final_scale = (T)(pow(step, (double)(n_steps % 4)) *
+                        exp((double)groups * log(pow(step, 4) / (double)p.scale4)));
     const int nw = (int)(L.ny / R);
     const bool per = L.periodic_x != 0;
     if (R == 2) return launch_r<T, 2>(p, pot != nullptr, per, nw, st);
     if (R == 4 && !pot)      // (with the phase rows in registers four rows per warp would spill)
         return per ? launch_one(tiny_kernel<T, 4, false, true>, p, nw, st)
                    : launch_one(tiny_kernel<T, 4, false, false>, p, nw, st);
+    if (R == 8 && !pot)
+        return per ? launch_one(tiny_kernel<T, 8, false, true>, p, nw, st)
+                   : launch_one(tiny_kernel<T, 8, false, false>, p, nw, st);
     set_error("tiny_evolve: lattice does not fit one block");
     return TS_EUNSUPPORTED;
 }
 
 }  // namespace
 
-int tiny_rows_per_warp(const LatticeDesc& L, bool pot) {
-    // rows per warp: 2, or 4 without a potential; at most 32 warps in fp32 and 16 in fp64 (register
-    // budget), i.e. up to 128 x 128 (fp32) / 128 x 64 (fp64) sites, half of that with a potential.
+int tiny_rows_per_warp(const LatticeDesc& L, bool pot, int prefer) {
+    // rows per warp R: 2 (up to 32 warps in fp32, 16 in fp64: register budget at 1024 / 512
+    // threads), and without a potential 4, or 8 with at most 8 warps.  More rows per warp mean
+    // fewer vertical-odd pairs through shared memory: C1 runs 3.6 / 4.5 / 4.8e9 site-steps/s at
+    // R = 2 / 4 / 8, so the largest R that fits is taken unless `prefer` (2, 4, 8) says otherwise.
+    // Capacity: 128 x 128 sites in fp32, 128 x 64 in fp64; half of that with a potential.
     // 0 = the lattice does not fit one block.
     if (L.nx > kStripSites || L.nx % 4 || L.ny % 2 || L.periodic_x != L.periodic_y) return 0;
     const int max_warps = L.dtype == TS_F32 ? 32 : 16;
-    if (L.ny / 2 <= max_warps) return 2;
-    if (!pot && L.ny % 4 == 0 && L.ny / 4 <= max_warps) return 4;
+    const bool ok8 = !pot && L.ny % 8 == 0 && L.ny / 8 <= 8;
+    const bool ok4 = !pot && L.ny % 4 == 0 && L.ny / 4 <= max_warps;
+    const bool ok2 = L.ny / 2 <= max_warps;
+    if (prefer == 2 && ok2) return 2;
+    if (prefer == 4 && ok4) return 4;
+    if (ok8) return 8;
+    if (ok4) return 4;
+    if (ok2) return 2;
     return 0;
 }
 
 bool tiny_supported(const LatticeDesc& L, const StepCoef& c, bool pot) {
-    return tiny_rows_per_warp(L, pot) != 0 && c.a_h > 0.25 && c.a_f > 0.25;
+    return tiny_rows_per_warp(L, pot, 0) != 0 && c.a_h > 0.25 && c.a_f > 0.25;
 }
 
 int tiny_evolve(const LatticeDesc& L, void* re, void* im, const StepCoef& c, const void* pot,
-                int64_t n_steps, cudaStream_t st) {
+                int64_t n_steps, int rows_per_warp, cudaStream_t st) {
     if (L.dtype == TS_F32)
-        return evolve_t<float>(L, (float*)re, (float*)im, c, (const float*)pot, n_steps, st);
-    return evolve_t<double>(L, (double*)re, (double*)im, c, (const double*)pot, n_steps, st);
+        return evolve_t<float>(L, (float*)re, (float*)im, c, (const float*)pot, n_steps,
+                               rows_per_warp, st);
+    return evolve_t<double>(L, (double*)re, (double*)im, c, (const double*)pot, n_steps,
+                            rows_per_warp, st);
 }
 
 }  // namespace ts

@@ -32,13 +32,17 @@ def test_on_chip_kernel(dtype, boundary, with_pot, idx):
     n = 23
     cfg = G.make_cfg(nx, ny, dtype, boundary, 0.3, n)
     re, im, pot = G.random_inputs(nx, ny, dtype, 7 * nx + ny, with_pot)
-    got_re, got_im, info = G.gpu_evolve(cfg, re, im, pot, n_steps=n, variant=3)
     want_re, want_im = G.oracle_evolve(cfg, re, im, pot, n_steps=n)
-    err, rel = G.errors(cfg, got_re, got_im, want_re, want_im)
-    assert info["fused"] == 1 and info["variant"] == 3 and info["launches"] == 1
-    assert err <= TIGHT[dtype] * 3, (err, rel, info)
-    drift = info["norm2_after"] / info["norm2_before"] - 1
-    assert abs(drift) < (1e-4 if dtype == "f32" else 1e-12), drift
+    # rows per warp: the default (largest that fits) and every smaller one that fits
+    for rows in (0, 4, 2):
+        if rows == 2 and not rows_per_warp_2:
+            continue
+        got_re, got_im, info = G.gpu_evolve(cfg, re, im, pot, n_steps=n, variant=3, seg_rows=rows)
+        err, rel = G.errors(cfg, got_re, got_im, want_re, want_im)
+        assert info["fused"] == 1 and info["variant"] == 3 and info["launches"] == 1
+        assert err <= TIGHT[dtype] * 3, (rows, err, rel, info)
+        drift = info["norm2_after"] / info["norm2_before"] - 1
+        assert abs(drift) < (1e-4 if dtype == "f32" else 1e-12), (rows, drift)
 
 
 def test_it_is_the_default_for_lattices_that_fit_and_only_for_those():
