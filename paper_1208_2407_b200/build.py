@@ -22,7 +22,7 @@ UNITS = [("ts_api.cu", "ts_api", []), ("ts_generic.cu", "ts_generic", []),
          ("ts_stream.cu", "ts_stream_f64", ["-DTS_STREAM_TU=64"])]
 HEADERS = [CSRC / "ts_internal.h", CSRC / "ts_rows.cuh", INCLUDE / "ts.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "--use_fast_math=false"]
+              "-Xcompiler", "-fPIC"]
 
 
 def _nvcc() -> str:
@@ -44,7 +44,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     if not force and not needs_build():
         return LIB
     nvcc = _nvcc()
-    flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
+    flags = list(NVCC_FLAGS)
     if verbose:
         flags += ["-Xptxas", "-v"]
     objs = []

@@ -18,7 +18,6 @@
 #include <math.h>
 
 #include "ts_internal.h"
-#include "ts_internal.h"
 #include "ts_rows.cuh"
 
 namespace ts {

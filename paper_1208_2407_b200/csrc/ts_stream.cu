@@ -484,10 +484,7 @@ int launch(const StreamParams<T>& p, cudaStream_t st) {
     const size_t smem = (size_t)kWarps * p.nst * (SLOTB + 8);
     // register budget: the ring (64 KB per block) admits 3 blocks per SM anyway, so fp32 gets 168
     // registers from S = 3 on (128 below); fp64 3 or 2 blocks (255)
-#ifndef TS_MINB_F32
-#define TS_MINB_F32 (S <= 2 ? 4 : 3)
-#endif
-    constexpr int MINB = sizeof(T) == 4 ? TS_MINB_F32 : (S <= 2 ? 3 : 2);
+    constexpr int MINB = sizeof(T) == 4 ? (S <= 2 ? 4 : 3) : (S <= 2 ? 3 : 2);
     auto kern = stream_kernel<T, S, PM, BND, MINB>;
     // the opt-in for > 48 KB of dynamic shared memory is a per-device, per-kernel attribute:
     // remembered per instantiation and device (atomics: plans on different threads may race here,

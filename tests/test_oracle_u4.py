@@ -99,3 +99,49 @@ def test_reversibility_and_norm():
     conj = lambda P: (P[0], -P[1])
     oracle.evolve_u4(re, im, -0.3, pot_p=conj(pp), pot_q=conj(pq), periodic=True, n_steps=5)
     assert np.abs(re - re0).max() < 1e-13 and np.abs(im - im0).max() < 1e-13
+
+
+# ---- time-dependent potential (the Hamiltonian may depend on time) ------------------
+# oracle.evolve_tdep is the checker of ts_evolve_tdep; what it adds to the pinned single step is the
+# ORDER in which the list is consumed and the potential-free (None) entry.
+
+@pytest.mark.parametrize("nx,ny,periodic", [(6, 4, True), (5, 3, False), (4, 6, False)])
+def test_tdep_equals_ordered_dense_product_and_order_matters(nx, ny, periodic):
+    theta = 0.45
+    c = (math.cos(theta / 2), math.sin(theta / 2), math.cos(theta), math.sin(theta))
+    rng = np.random.default_rng(17)
+    Vs = [rng.uniform(-2, 2, (ny, nx)) for _ in range(3)]
+    order = [0, 1, None, 2, 1]                     # step k uses Vs[order[k]]; None: 7-stage step
+    pots_k = [None if k is None else (np.cos(Vs[k]), -np.sin(Vs[k])) for k in order]
+    re, im = rand_state(ny, nx, 23)
+    v = to_vec(re, im)
+    for k in order:                                # applied left to right = first step first
+        v = step_unitary(nx, ny, periodic, theta, None if k is None else Vs[k], 1.0) @ v
+    w_re, w_im = from_vec(v, ny, nx)
+    g_re, g_im = re.copy(), im.copy()
+    oracle.evolve_tdep(g_re, g_im, *c, pots_k, periodic=periodic)
+    assert np.abs(g_re - w_re).max() < 1e-13 and np.abs(g_im - w_im).max() < 1e-13
+    # the reversed list is a different operator: the pin above would not pass for it
+    r_re, r_im = re.copy(), im.copy()
+    oracle.evolve_tdep(r_re, r_im, *c, pots_k[::-1], periodic=periodic)
+    assert max(np.abs(r_re - w_re).max(), np.abs(r_im - w_im).max()) > 1e-3
+    # dropping the potential-free step is a different operator as well
+    d_re, d_im = re.copy(), im.copy()
+    oracle.evolve_tdep(d_re, d_im, *c, [p for p in pots_k if p is not None], periodic=periodic)
+    assert max(np.abs(d_re - w_re).max(), np.abs(d_im - w_im).max()) > 1e-3
+
+
+def test_tdep_with_one_repeated_array_is_evolve():
+    nx, ny, theta, n = 6, 4, 0.3, 4
+    c = (math.cos(theta / 2), math.sin(theta / 2), math.cos(theta), math.sin(theta))
+    V = np.random.default_rng(2).uniform(-3, 3, (ny, nx))
+    pot = (np.cos(V), -np.sin(V))
+    re, im = rand_state(ny, nx, 4)
+    a_re, a_im = re.copy(), im.copy()
+    oracle.evolve_tdep(a_re, a_im, *c, [pot] * n, periodic=True)
+    v = np.linalg.matrix_power(step_unitary(nx, ny, True, theta, V, 1.0), n) @ to_vec(re, im)
+    w_re, w_im = from_vec(v, ny, nx)
+    assert np.abs(a_re - w_re).max() < 1e-13 and np.abs(a_im - w_im).max() < 1e-13
+    e_re, e_im = re.copy(), im.copy()
+    oracle.evolve_tdep(e_re, e_im, *c, [], periodic=True)      # empty list: identity
+    assert np.array_equal(e_re, re) and np.array_equal(e_im, im)
