@@ -15,12 +15,13 @@ INCLUDE = PKG.parent / "include"
 LIB = PKG / "libts.so"
 # (source, object stem, extra flags); ts_stream.cu is compiled once per dtype so that its kernel
 # instantiations build in parallel
-SOURCES = ["ts_api.cu", "ts_generic.cu", "ts_fused.cu", "ts_stream.cu", "ts_tiny.cu"]
+SOURCES = ["ts_api.cu", "ts_generic.cu", "ts_fused.cu", "ts_stream.cu", "ts_tiny.cu", "ts_axis.cu"]
 UNITS = [("ts_api.cu", "ts_api", []), ("ts_generic.cu", "ts_generic", []),
          ("ts_fused.cu", "ts_fused", []), ("ts_tiny.cu", "ts_tiny", []),
+         ("ts_axis.cu", "ts_axis", []),
          ("ts_stream.cu", "ts_stream_f32", ["-DTS_STREAM_TU=32"]),
          ("ts_stream.cu", "ts_stream_f64", ["-DTS_STREAM_TU=64"])]
-HEADERS = [CSRC / "ts_internal.h", CSRC / "ts_rows.cuh", INCLUDE / "ts.h"]
+HEADERS = [CSRC / "ts_internal.h", CSRC / "ts_rows.cuh", CSRC / "ts_tma.cuh", INCLUDE / "ts.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 

@@ -36,9 +36,10 @@ struct ts_plan {
     void* sep_pot;            // separable phase written out as planes (paths without mode 2)
     cudaStream_t own_stream;
     // options
-    int64_t opt_path, opt_fuse, opt_seg, opt_variant, opt_slots;
+    int64_t opt_path, opt_fuse, opt_seg, opt_variant, opt_slots, opt_chain;
     // info on the last ts_evolve
     int64_t info_fused, info_fuse, info_passes, info_launches, info_seg, info_variant;
+    int64_t info_chain_x, info_chain_y;
 };
 
 namespace {
@@ -145,8 +146,11 @@ int ts_plan_set_option(ts_plan* plan, const char* name, int64_t value) {
         if (value < 0 || value % 2) return fail(TS_EINVAL, "seg_rows must be even and >= 0");
         plan->opt_seg = value;
     } else if (!strcmp(name, "variant")) {
-        if (value < 0 || value > 3) return fail(TS_EINVAL, "variant must be 0, 1, 2 or 3");
+        if (value < 0 || value > 4) return fail(TS_EINVAL, "variant must be 0 .. 4");
         plan->opt_variant = value;
+    } else if (!strcmp(name, "chain")) {
+        if (value < 0 || value > 64) return fail(TS_EINVAL, "chain out of range");
+        plan->opt_chain = value;
     } else if (!strcmp(name, "ring_slots")) {
         if (value < 0 || value > 64) return fail(TS_EINVAL, "ring_slots out of range");
         plan->opt_slots = value;
@@ -164,6 +168,8 @@ int ts_plan_get_info(const ts_plan* plan, const char* name, int64_t* out) {
     else if (!strcmp(name, "launches")) *out = plan->info_launches;
     else if (!strcmp(name, "seg_rows")) *out = plan->info_seg;
     else if (!strcmp(name, "variant")) *out = plan->info_variant;
+    else if (!strcmp(name, "chain_x")) *out = plan->info_chain_x;
+    else if (!strcmp(name, "chain_y")) *out = plan->info_chain_y;
     else return fail(TS_EINVAL, "unknown info name");
     return TS_OK;
 }
@@ -225,24 +231,82 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
         if (u.a_h * v.a_h - u.b_h * v.b_h <= 0.25) can_v1 = can_stream = false;
     }
     const bool can_fuse = can_v1 || can_stream;
+    // steps without a potential factorise into a row chain and a column chain (ts_axis.cu)
+    ts::StepCoef axis_pat[8];
+    bool can_axis = !any_pot && period <= 8;
+    if (can_axis) {
+        for (int k = 0; k < period; ++k) axis_pat[k] = pat[k].c;
+        can_axis = ts::axis_supported(L, axis_pat, period);
+    }
     int rc = check_device(plan);
     if (rc != TS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
 
     plan->info_fused = plan->info_fuse = plan->info_passes = plan->info_launches = 0;
-    plan->info_seg = plan->info_variant = 0;
+    plan->info_seg = plan->info_variant = plan->info_chain_x = plan->info_chain_y = 0;
     if (n_repeat == 0) return TS_OK;
     if (period > 1 && n_repeat > (int64_t(1) << 56)) return fail(TS_EINVAL, "n_steps too large");
     const int64_t n_sub = n_repeat * period;
 
+    // ---- which path: every rejection comes before the first allocation or launch -----------------
     // tiny lattices: the whole evolution in one launch of the on-chip-resident kernel (uniform
     // steps, no or plane potential)
     const bool can_tiny = period == 1 && pat[0].ph.mode != 2 &&
                           ts::tiny_supported(L, pat[0].c, pat[0].ph.mode == 1);
-    if (plan->opt_variant == 3 && !can_tiny)
+    const int64_t variant = plan->opt_variant;
+    if (variant == 3 && !can_tiny)
         return fail(TS_EUNSUPPORTED, "the on-chip kernel takes uniform steps on lattices of at most "
                                      "128 x 128 (fp32) / 128 x 64 (fp64) sites, half with a potential");
-    if (can_tiny && plan->opt_path != 1 && (plan->opt_variant == 0 || plan->opt_variant == 3)) {
+    if (variant == 4 && !can_axis)
+        return fail(TS_EUNSUPPORTED, "the axis-split path takes steps without a potential, nx % 4 == 0, "
+                                     "even ny, cos of every sweep angle > 0.25");
+    if (plan->opt_path == 2 && !can_fuse && !can_axis)
+        return fail(TS_EUNSUPPORTED,
+                    "fused kernel needs nx % 4 == 0, even ny and cos(theta) > 0.25");
+    if (variant == 2 && !can_stream)
+        return fail(TS_EUNSUPPORTED, "the TMA ring kernel needs nx >= 128 on a lattice that is periodic in x");
+    if (variant == 1 && !can_v1)
+        return fail(TS_EUNSUPPORTED, "the register-prefetch kernel needs one boundary type on both axes");
+    const bool generic = plan->opt_path == 1 || (!can_fuse && !can_axis);
+    const bool use_axis = !generic && can_axis && (variant == 0 || variant == 4);
+    const bool use_tiny = !generic && !use_axis && can_tiny && (variant == 0 || variant == 3);
+    const bool use_stream = !generic && !use_axis && !use_tiny && can_stream && variant != 1;
+    if (!generic && !use_axis && !use_tiny && !can_fuse)
+        return fail(TS_EUNSUPPORTED, "the requested kernel variant does not take this lattice");
+    const bool expand_sep = any_sep && !use_stream;
+    if (expand_sep && period != 1)
+        return fail(TS_EUNSUPPORTED, "separable phases of a multi-sub-step pattern need the TMA ring kernel");
+    int S = 0, s_max = 0;
+    if (!generic && !use_axis && !use_tiny) {
+        S = plan->opt_fuse ? (int)plan->opt_fuse
+                           : (any_sep && use_stream ? ts::stream_default_steps_sep(L)
+                                                    : ts::fused_default_steps(L, any_pot));
+        s_max = use_stream ? ts::stream_max_steps(L, any_pot) : 4;
+        if (S > s_max) {
+            if (plan->opt_fuse)
+                return fail(TS_EUNSUPPORTED, "fuse_steps > 4 needs the TMA ring kernel, fp32, no potential");
+            S = s_max;
+        }
+    }
+
+    if (use_axis) {
+        if (ts::axis_needs_scratch(L)) {
+            rc = ensure_alloc(&plan->scratch_re, plane_bytes);
+            if (rc == TS_OK) rc = ensure_alloc(&plan->scratch_im, plane_bytes);
+            if (rc != TS_OK) return rc;
+        }
+        ts::AxisInfo ai;
+        rc = ts::axis_evolve(L, psi_re, psi_im, plan->scratch_re, plan->scratch_im, axis_pat, period,
+                             n_sub, (int)plan->opt_chain, (int)plan->opt_seg, (int)plan->opt_slots,
+                             st, &ai);
+        plan->info_launches = ai.launches;
+        if (rc != TS_OK) return rc;
+        plan->info_fused = 1; plan->info_passes = ai.passes; plan->info_seg = ai.seg_rows;
+        plan->info_chain_x = ai.chain_x; plan->info_chain_y = ai.chain_y;
+        plan->info_fuse = ai.chain_y; plan->info_variant = 4;
+        return TS_OK;
+    }
+    if (use_tiny) {
         rc = ts::tiny_evolve(L, psi_re, psi_im, pat[0].c, pat[0].ph.planes, n_repeat,
                              (int)plan->opt_seg, st);     // "seg_rows" = rows per warp here
         if (rc != TS_OK) return rc;
@@ -250,16 +314,10 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
         plan->info_launches = 1; plan->info_seg = L.ny; plan->info_variant = 3;
         return TS_OK;
     }
-    if (plan->opt_path == 2 && !can_fuse)
-        return fail(TS_EUNSUPPORTED,
-                    "fused kernel needs nx % 4 == 0, even ny and cos(theta) > 0.25");
-    const bool use_stream_early = can_stream && plan->opt_variant != 1 && plan->opt_path != 1 &&
-                                  can_fuse;
     // separable factors are consumed directly only by the TMA ring kernel; every other path gets
     // them written out as planes (one array: period-1 patterns only)
     SubStep expanded;
-    if (any_sep && !use_stream_early) {
-        if (period != 1) return fail(TS_EUNSUPPORTED, "separable phases of a multi-sub-step pattern need the TMA ring kernel");
+    if (expand_sep) {
         rc = ensure_alloc(&plan->sep_pot, 2 * plane_bytes);
         if (rc != TS_OK) return rc;
         rc = ts::expand_separable(L, pat[0].ph.px, pat[0].ph.py, plan->sep_pot, st);
@@ -269,7 +327,7 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
         expanded.ph = ts::Phase{1, plan->sep_pot, nullptr, nullptr};
         pat = &expanded;
     }
-    if (plan->opt_path == 1 || !can_fuse) {
+    if (generic) {
         const int64_t l0 = plan->info_launches;
         if (period == 1) {
             rc = ts::generic_evolve(L, psi_re, psi_im, pat[0].c, pat[0].ph.planes, n_repeat, st,
@@ -291,20 +349,6 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
     if (rc == TS_OK) rc = ensure_alloc(&plan->scratch_im, plane_bytes);
     if (rc != TS_OK) return rc;
 
-    if (plan->opt_variant == 2 && !can_stream)
-        return fail(TS_EUNSUPPORTED, "the TMA ring kernel needs nx >= 128 on a lattice that is periodic in x");
-    if (plan->opt_variant == 1 && !can_v1)
-        return fail(TS_EUNSUPPORTED, "the register-prefetch kernel needs one boundary type on both axes");
-    const bool use_stream = can_stream && plan->opt_variant != 1;
-    int S = plan->opt_fuse ? (int)plan->opt_fuse
-                           : (any_sep && use_stream ? ts::stream_default_steps_sep(L)
-                                                    : ts::fused_default_steps(L, any_pot));
-    const int s_max = use_stream ? ts::stream_max_steps(L, any_pot) : 4;
-    if (S > s_max) {
-        if (plan->opt_fuse)
-            return fail(TS_EUNSUPPORTED, "fuse_steps > 4 needs the TMA ring kernel, fp32, no potential");
-        S = s_max;
-    }
     // resident blocks per SM of the kernel that will run: the ring with phase planes is twice as
     // large; fp64 pipelines beyond S = 2 take 255 registers
     const bool planes = any_pot && !(any_sep && use_stream);

@@ -92,4 +92,21 @@ int expand_separable(const LatticeDesc& L, const void* px, const void* py, void*
                      cudaStream_t st);
 int fused_default_steps(const LatticeDesc& L, bool pot);
 
+
+// ---- axis-split path for steps without a potential (ts_axis.cu) ------------------------------------
+// U2^n = (row chain) x (column chain): whole lines resident in a warp's registers where they fit
+// (one launch per axis for ALL sub-steps, in place), else windowed rows / pipelined columns with up
+// to 16 sub-steps per pass (out of place, ping-pong with the scratch planes).
+struct AxisInfo {
+    int64_t passes, launches, chain_x, chain_y, seg_rows;
+};
+bool axis_supported(const LatticeDesc& L, const StepCoef* pat, int period);
+bool axis_needs_scratch(const LatticeDesc& L);
+int axis_default_chain(const LatticeDesc& L);
+// psi <- (U2(pat[period-1]) ... U2(pat[0]))^(n_sub / period) psi, n_sub sub-steps in pattern order.
+// chain: sub-steps per windowed / pipelined pass (0 = default); seg_rows, nst: 0 = default.
+int axis_evolve(const LatticeDesc& L, void* psi_re, void* psi_im, void* scr_re, void* scr_im,
+                const StepCoef* pat, int period, int64_t n_sub, int chain, int seg_rows, int nst,
+                cudaStream_t st, AxisInfo* info);
+
 }  // namespace ts

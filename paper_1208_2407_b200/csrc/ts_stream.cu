@@ -21,11 +21,13 @@
 
 #include "ts_internal.h"
 #include "ts_rows.cuh"
+#include "ts_tma.cuh"
 
 namespace ts {
 namespace {
 
 using namespace rows;
+using namespace tma;
 
 constexpr int kWarps = 4;
 constexpr int kMaxDevices = 64;
@@ -67,65 +69,6 @@ struct StreamParams {
     T sec_ox[TS_MAX_FUSE];   // regrouping brings together, composed from the HALF coefficients
     T out_scale;             // product of all deferred cosines of the pass
 };
-
-// ---- PTX: mbarrier + bulk async copy (TMA) -------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
-}
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_fence_init() {
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "WAIT_LOOP:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra WAIT_DONE;\n\t"
-        "bra WAIT_LOOP;\n\t"
-        "WAIT_DONE:\n\t"
-        "}" ::"r"(bar), "r"(parity)
-        : "memory");
-}
-// global -> shared bulk copy; bytes % 16 == 0, both addresses 16-byte aligned
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes,
-                                         uint32_t bar) {
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-        ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
-        : "memory");
-}
-
-__device__ __forceinline__ void lds4(uint32_t addr, float (&v)[4]) {
-    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
-                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]) : "r"(addr));
-}
-__device__ __forceinline__ void lds4(uint32_t addr, double (&v)[4]) {
-    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[0]), "=d"(v[1]) : "r"(addr));
-    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[2]), "=d"(v[3]) : "r"(addr + 16));
-}
-
-// one lane per warp, known to the compiler as a single active lane (no per-lane issue loops)
-__device__ __forceinline__ bool elect_one() {
-    uint32_t pred;
-    asm volatile(
-        "{\n\t"
-        ".reg .pred P;\n\t"
-        "elect.sync _|P, 0xffffffff;\n\t"
-        "selp.u32 %0, 1, 0, P;\n\t"
-        "}" : "=r"(pred));
-    return pred != 0;
-}
 
 template <typename T>
 struct StreamCtx {
@@ -175,9 +118,10 @@ __device__ __forceinline__ void stream_stage(const StreamParams<T>& p, const Str
             // py is indexed by the GLOBAL row: py_off = first row of a slab (0 for a whole
             // lattice), py_n = global height, py_wrap = the global lattice is periodic in y
             int ylo = yj - 1 + p.py_off, yhi = yj + p.py_off;
-            if (p.py_wrap) {   // |excursion| < py_n: one conditional add each way, no loop
-                ylo += ylo < 0 ? p.py_n : 0;  ylo -= ylo >= p.py_n ? p.py_n : 0;
-                yhi += yhi < 0 ? p.py_n : 0;  yhi -= yhi >= p.py_n ? p.py_n : 0;
+            if (p.py_wrap) {   // warm-up rows reach 2S + 1 rows above row 0: further than a
+                               // very short ring is long, hence the looped form
+                ylo = wrap_index(ylo, p.py_n);
+                yhi = wrap_index(yhi, p.py_n);
             }
             else { ylo = min(max(ylo, 0), p.py_n - 1); yhi = min(max(yhi, 0), p.py_n - 1); }
             sep_phase_row(h, c.pxr, c.pxi, __ldg(p.py_re + ylo), __ldg(p.py_im + ylo));
@@ -299,16 +243,6 @@ stream_kernel(const StreamParams<T> p) {
     c.e.dn = !PERX && (xb + 4 == p.nx || xb + 4 == 0);
     c.ring = smem_u32(smem_raw) + warp * NST * SLOTB;
     c.lane_off = lane * 4 * sizeof(T);
-    if (PM == 2) {
-        // the lane's four columns (wrapped when periodic; 1 + 0i on ghost columns, which hold zeros)
-        const int xw = PERX ? wrap_index(xb, p.nx) : xb;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const bool ok = PERX || (xb >= 0 && xb < p.nx);
-            c.pxr[i] = ok ? __ldg(p.px_re + xw + i) : T(1);
-            c.pxi[i] = ok ? __ldg(p.px_im + xw + i) : T(0);
-        }
-    }
     const uint32_t bars = smem_u32(smem_raw) + kWarps * NST * SLOTB + warp * NST * 8;
     const bool store_ok = (4 * lane >= p.halo) && (4 * lane < kStripSites - p.halo) && (xb < p.nx);
 
@@ -345,12 +279,24 @@ stream_kernel(const StreamParams<T> p) {
     __syncwarp();
     // Programmatic dependent launch: the passes of one ts_evolve are launched with stream
     // serialisation relaxed, so this grid's blocks may be scheduled (and get here) while the
-    // previous pass is still draining; nothing the previous pass wrote has been touched yet
-    // (px / the kernel parameters are inputs), and nothing is written before this point.
+    // previous pass is still draining; no global memory has been read and nothing has been
+    // written before this point (the separable phase vectors, too, are read after the wait: the
+    // caller may have produced them with a kernel just before on the same stream).
     // griddepcontrol.wait returns once the previous grid has completed and its writes are visible;
     // launch_dependents lets the next pass start its own prologue as early as possible.
     asm volatile("griddepcontrol.wait;" ::: "memory");
     asm volatile("griddepcontrol.launch_dependents;");
+
+    if (PM == 2) {
+        // the lane's four columns (wrapped when periodic; 1 + 0i on ghost columns, which hold zeros)
+        const int xw = PERX ? wrap_index(xb, p.nx) : xb;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const bool ok = PERX || (xb >= 0 && xb < p.nx);
+            c.pxr[i] = ok ? __ldg(p.px_re + xw + i) : T(1);
+            c.pxi[i] = ok ? __ldg(p.px_im + xw + i) : T(0);
+        }
+    }
 
     // running row of the next fetch (warp-uniform): rows (fy, fy+1), element offset foff
     int fy = PERY ? wrap_index(y_in0, p.ny) : y_in0;

@@ -14,7 +14,7 @@ def torch_dtype(cfg):
 
 
 def gpu_evolve(cfg, re_np, im_np, pot_np=None, n_steps=None, path=0, fuse=0, seg_rows=0,
-               coeffs=None, variant=0, ring_slots=0):
+               coeffs=None, variant=0, ring_slots=0, chain=0):
     """Upload, ts_evolve, download.  Returns (re, im, info dict)."""
     import torch
     from paper_1208_2407_b200.binding import Plan
@@ -25,6 +25,7 @@ def gpu_evolve(cfg, re_np, im_np, pot_np=None, n_steps=None, path=0, fuse=0, seg
     plan.set_option("seg_rows", seg_rows)
     plan.set_option("variant", variant)
     plan.set_option("ring_slots", ring_slots)
+    plan.set_option("chain", chain)
     re = torch.from_numpy(np.ascontiguousarray(re_np)).to(dev)
     im = torch.from_numpy(np.ascontiguousarray(im_np)).to(dev)
     pot = None if pot_np is None else torch.from_numpy(np.ascontiguousarray(pot_np)).to(dev)
@@ -35,7 +36,7 @@ def gpu_evolve(cfg, re_np, im_np, pot_np=None, n_steps=None, path=0, fuse=0, seg
     torch.cuda.synchronize()
     n2_after = plan.norm(re, im)
     info = {k: plan.info(k) for k in ("fused", "fuse_steps", "passes", "launches", "seg_rows",
-                                     "variant")}
+                                     "variant", "chain_x", "chain_y")}
     info["norm2_before"], info["norm2_after"] = n2_before, n2_after
     out = re.cpu().numpy(), im.cpu().numpy()
     plan.destroy()

@@ -44,8 +44,13 @@ def test_full_lattice_configs(name):
     assert abs(info["norm2_before"] - 1) < 1e-5
 
 
-def _windows(cfg, S, seg):
-    wi = 128 - 2 * ((2 * S + 3) // 4 * 4)
+def _windows(cfg, S, seg, variant=2):
+    # x seams: interior width of a strip of the 2-D streaming kernel, or of a row window of the
+    # axis-split path (1024 / 512 sites less a halo of 2 per chained sub-step, in fours)
+    if variant == 4:
+        wi = (1024 if cfg.dtype == "f32" else 512) - 2 * ((2 * S + 3) // 4 * 4)
+    else:
+        wi = 128 - 2 * ((2 * S + 3) // 4 * 4)
     nx, ny = cfg.nx, cfg.ny
     rng = np.random.default_rng(7)
     wins = [
@@ -97,7 +102,9 @@ def _run_periodic_config(cfg, sep=False):
     S, seg = max(1, plan.info("fuse_steps")), max(2, plan.info("seg_rows"))
     S = S if cfg.n_steps >= S else cfg.n_steps
 
-    wins = _windows(cfg, plan.info("fuse_steps") or 2, seg)
+    variant = plan.info("variant")
+    wins = _windows(cfg, (plan.info("chain_x") if variant == 4 else plan.info("fuse_steps")) or 2,
+                    seg, variant)
     margin = 2 * cfg.n_steps + 2
     cut = {}
     for (x0, y0, w, h) in wins:       # cut the INPUT windows out before evolving in place
@@ -204,7 +211,12 @@ def test_C4_size_fourth_order_eigenstate():
     assert ph == 0.0 and ph_x != 0.0
     rel = max(float((re - ref).abs().max()), float(im.abs().max())) / amp
     print(f"\n[C4-size U4 eigenstate sx=1 sy=0] rel err {rel:.3e}  passes={plan.info('passes')}")
-    assert plan.info("fused") == 1 and plan.info("passes") == math.ceil(5 * n / 6)
+    assert plan.info("fused") == 1
+    if plan.info("variant") == 4:       # row chain + column chain, chain_x / chain_y sub-steps per pass
+        assert plan.info("passes") == (math.ceil(5 * n / plan.info("chain_x")) +
+                                       math.ceil(5 * n / plan.info("chain_y")))
+    else:
+        assert plan.info("passes") == math.ceil(5 * n / 6)
     assert rel < 2e-5
     # and a state whose phase does not cancel: sx = sy = 0 (uniform), phase 4 n theta
     re.fill_(amp); im.zero_()
@@ -245,3 +257,89 @@ def test_full_size_periodic_eigenstates(name, sx, sy):
     assert plan.info("fused") == 1
     assert rel < (2e-5 if cfg.dtype == "f32" else 1e-13)
     plan.destroy()
+
+
+# ---- every element of a full-size lattice against the full oracle ----------------------------------
+def _full_lattice_check(cfg, n_steps, option_sets, sep=False):
+    """Every element of the lattice against the full oracle for n_steps steps, once per set of plan
+    options (the oracle runs once).  Inputs are built on the device (bit-identical to the numpy
+    recipe) and downloaded for the oracle."""
+    import torch
+    from paper_1208_2407_b200.binding import Plan
+    dev = torch.device("cuda:0")
+    re0, im0, _ = inputs.device_state(cfg, dev)
+    pot = inputs.device_pot(cfg, dev)
+    c = cfg.coeffs()
+    wre = re0.cpu().numpy().astype(np.float64)
+    wim = im0.cpu().numpy().astype(np.float64)
+    wpot = None
+    if pot is not None:
+        wpot = (pot[0].cpu().numpy().astype(np.float64), pot[1].cpu().numpy().astype(np.float64))
+    oracle.evolve(wre, wim, *c, pot=wpot, periodic=cfg.periodic, n_steps=n_steps)
+    del wpot
+    scale = max(np.abs(wre).max(), np.abs(wim).max())
+    out = []
+    for opts in option_sets:
+        plan = Plan(cfg.nx, cfg.ny, G.torch_dtype(cfg), cfg.boundary)
+        for k, v in opts.items():
+            plan.set_option(k, v)
+        re, im = re0.clone(), im0.clone()
+        n0 = plan.norm(re, im)
+        plan.evolve(re, im, *c, pot_phase=pot, n_steps=n_steps)
+        torch.cuda.synchronize()
+        n1 = plan.norm(re, im)
+        info = {k: plan.info(k) for k in ("fused", "fuse_steps", "passes", "seg_rows", "variant")}
+        err = 0.0
+        rows = 2048
+        for y0 in range(0, cfg.ny, rows):       # compare in slabs: no second full-size host copy
+            gr = re[y0:y0 + rows].cpu().numpy().astype(np.float64)
+            gi = im[y0:y0 + rows].cpu().numpy().astype(np.float64)
+            err = max(err, np.abs(gr - wre[y0:y0 + rows]).max(), np.abs(gi - wim[y0:y0 + rows]).max())
+        plan.destroy()
+        del re, im
+        print(f"\n[{cfg.name} full lattice, {n_steps} steps, options {opts}] max-abs err {err:.3e}  "
+              f"rel {err / scale:.3e}  norm drift {n1 / n0 - 1:+.3e}  {info}")
+        out.append((err, err / scale, n1 / n0 - 1, info))
+    return out
+
+
+@pytest.mark.slow
+def test_C4_full_lattice_short():
+    """16384^2 fp32 periodic, 24 steps, EVERY element against the full oracle (about 20 s of oracle
+    time, 9 GB of host memory): default plan options (the path bench.py times) and the 2-D
+    streaming kernel at its default S = 6 (four passes)."""
+    import psutil
+    if psutil.virtual_memory().available < 14e9:
+        pytest.skip("needs ~12 GB of host memory")
+    cfg = inputs.CONFIGS["C4"]
+    res = _full_lattice_check(cfg, 24, [{}, {"variant": 2}])
+    for err, rel, drift, info in res:
+        assert info["fused"] == 1
+        assert err <= G.tol(cfg) and rel <= 2e-5 and abs(drift) < 1e-5, (err, rel, drift, info)
+    assert res[1][3]["variant"] == 2 and res[1][3]["fuse_steps"] == 6 and res[1][3]["passes"] == 4
+
+
+@pytest.mark.slow
+def test_C5_recipe_8192_full_lattice_short():
+    """The C5 recipe (fp64, periodic, harmonic trap as phase planes) on 8192^2 -- the full C5 oracle
+    needs 34 GB of host memory -- with default options, 12 steps, every element."""
+    cfg = inputs.scaled(inputs.CONFIGS["C5"], 8192, 8192, 12)
+    (err, rel, drift, info), = _full_lattice_check(cfg, 12, [{}])
+    assert info["fused"] == 1 and info["variant"] == 2
+    assert err <= G.tol(cfg) and rel <= 1e-11 and abs(drift) < 1e-12, (err, rel, drift, info)
+
+
+@pytest.mark.parametrize("recipe,opts", [("C4", {}), ("C4", {"variant": 2}), ("C3", {}), ("C5", {})])
+def test_2048_default_options_full_lattice(recipe, opts):
+    """Mid-size lattices with DEFAULT segment sizes and fusion depths (the small parity tests force
+    short segments): the C4 recipe (fp32 periodic, no potential) on the default path and on the
+    2-D streaming kernel, the C3 recipe (fp32 closed + trap) and the C5 recipe (fp64 periodic +
+    trap), 2048^2, 24 steps, every element against the full oracle."""
+    cfg = inputs.scaled(inputs.CONFIGS[recipe], 2048, 2048, 24)
+    (err, rel, drift, info), = _full_lattice_check(cfg, 24, [opts])
+    assert info["fused"] == 1 and info["seg_rows"] != 0
+    if recipe == "C4" and opts:
+        assert info["variant"] == 2
+    assert err <= G.tol(cfg), (err, info)
+    assert rel <= (2e-5 if cfg.dtype == "f32" else 1e-11), (rel, info)
+    assert abs(drift) < (1e-5 if cfg.dtype == "f32" else 1e-12)

@@ -63,6 +63,16 @@ def test_sep_stream_kernel(nx, ny, boundary, dtype, fuse):
         assert info["passes"] == math.ceil(9 / fuse)
 
 
+@pytest.mark.parametrize("nx,ny", [(256, 2), (256, 4), (128, 6), (256, 10)])
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("fuse", [0, 1, 2, 3, 4])
+def test_sep_periodic_rings_shorter_than_the_warm_up(nx, ny, dtype, fuse):
+    # the warm-up rows of the pipeline start 2S rows above row 0: on a periodic lattice with
+    # ny < 2S + 2 they wrap around the ring more than once, and py must be indexed accordingly
+    info = run(nx, ny, dtype, "periodic", 9, nx + 5 * ny + fuse, path=2, variant=2, fuse_steps=fuse)
+    assert info["fused"] == 1 and info["variant"] == 2
+
+
 @pytest.mark.parametrize("nx,ny,opts", [(64, 64, dict(path=2, variant=1)), (124, 34, dict(path=2, variant=1)),
                                         (129, 67, dict()), (256, 30, dict(path=1))])
 @pytest.mark.parametrize("dtype", ["f32", "f64"])

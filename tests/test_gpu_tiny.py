@@ -46,13 +46,14 @@ def test_on_chip_kernel(dtype, boundary, with_pot, idx):
 
 
 def test_it_is_the_default_for_lattices_that_fit_and_only_for_those():
+    # with a potential (without one the axis-split path is the default, tests/test_gpu_axis.py)
     cfg = G.make_cfg(64, 64, "f32", "closed", 0.01, 100)
-    re, im, _ = G.random_inputs(64, 64, "f32", 3, False)
-    _, _, info = G.gpu_evolve(cfg, re, im, None, n_steps=100)
+    re, im, pot = G.random_inputs(64, 64, "f32", 3, True)
+    _, _, info = G.gpu_evolve(cfg, re, im, pot, n_steps=100)
     assert info["variant"] == 3 and info["passes"] == 1
     cfg = G.make_cfg(128, 130, "f32", "closed", 0.01, 5)          # too tall: streaming kernel
-    re, im, _ = G.random_inputs(128, 130, "f32", 3, False)
-    _, _, info = G.gpu_evolve(cfg, re, im, None, n_steps=5)
+    re, im, pot = G.random_inputs(128, 130, "f32", 3, True)
+    _, _, info = G.gpu_evolve(cfg, re, im, pot, n_steps=5)
     assert info["variant"] == 2
     from paper_1208_2407_b200.binding import TsError, TS_EUNSUPPORTED
     with pytest.raises(TsError) as e:
@@ -61,8 +62,19 @@ def test_it_is_the_default_for_lattices_that_fit_and_only_for_those():
 
 
 def test_long_evolution_stays_in_range():
-    # the deferred cosines are multiplied in every step: 20000 steps at a large angle would
-    # otherwise leave the fp32 range (cos(0.45)^-7 per step)
+    # the deferred cosines are multiplied in every fourth step: thousands of steps at a large angle
+    # would otherwise leave the fp32 range (cos(0.45)^-7 per step).  Against the oracle: fp64 to
+    # rounding, fp32 to the rounding accumulated over 2000 steps of 7 sweeps.
+    for dtype, tol, drift_tol in (("f64", 1e-10, 1e-11), ("f32", 2e-3, 2e-3)):
+        cfg = G.make_cfg(32, 16, dtype, "periodic", 0.9, 2000)
+        re, im, _ = G.random_inputs(32, 16, dtype, 1, False)
+        got_re, got_im, info = G.gpu_evolve(cfg, re, im, None, n_steps=2000, variant=3)
+        want_re, want_im = G.oracle_evolve(cfg, re, im, None, n_steps=2000)
+        err, rel = G.errors(cfg, got_re, got_im, want_re, want_im)
+        assert info["variant"] == 3 and info["launches"] == 1
+        assert err < tol, (dtype, err, rel)
+        assert abs(info["norm2_after"] / info["norm2_before"] - 1) < drift_tol
+    # and 20000 steps in fp32 stay finite and normalised
     cfg = G.make_cfg(32, 16, "f32", "periodic", 0.9, 20000)
     re, im, _ = G.random_inputs(32, 16, "f32", 1, False)
     got_re, got_im, info = G.gpu_evolve(cfg, re, im, None, n_steps=20000, variant=3)
