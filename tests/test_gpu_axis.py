@@ -51,33 +51,43 @@ def test_resident_lines(dtype, boundary, idx, n_steps):
     assert info["chain_x"] == n_steps and info["chain_y"] == n_steps
 
 
-# rows longer than a warp holds (windows with a halo) and / or columns that are pipelined
-LONG = {"f32": [(2048, 128), (1152, 200), (64, 2048), (1280, 130), (3072, 1100), (4096, 66)],
-        "f64": [(1024, 128), (576, 200), (64, 1024), (640, 130), (1536, 1100)]}
+# lines shared by several warps of a block (2048 = 2 x 32 x 32, 1152 = 9 x 32 x 4, ...), rows that
+# fit no block and are cut into windows with a halo (1056 = 33 x 32, 20480, 528, 12288), columns
+# that are pipelined (130, 1100, 66 rows: no lane layout divides them)
+LONG = {"f32": [(2048, 128), (1152, 200), (64, 2048), (1280, 130), (3072, 1100), (4096, 66),
+                (1056, 200), (20480, 66), (16384, 16)],
+        "f64": [(1024, 128), (576, 200), (64, 1024), (640, 130), (1536, 1100), (528, 200),
+                (12288, 66), (8192, 16)]}
 
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 @pytest.mark.parametrize("boundary", ["closed", "periodic"])
-@pytest.mark.parametrize("idx", range(6))
-@pytest.mark.parametrize("chain", [0, 4, 7, 16])
-def test_windowed_rows_and_pipelined_columns(dtype, boundary, idx, chain):
+@pytest.mark.parametrize("idx", range(9))
+@pytest.mark.parametrize("chain", [0, 4, 7, 16, 24])
+def test_multi_warp_lines_windowed_rows_and_pipelined_columns(dtype, boundary, idx, chain):
     if idx >= len(LONG[dtype]):
         pytest.skip("no such shape for this dtype")
-    if dtype == "f64" and chain > 8:
-        pytest.skip("fp64 chains are at most 8 deep")
+    if dtype == "f64" and chain > 12:
+        pytest.skip("fp64 chains are at most 12 deep")
     nx, ny = LONG[dtype][idx]
     n_steps = 19
     cfg = G.make_cfg(nx, ny, dtype, boundary, 0.3, n_steps)
     info = check(cfg, n_steps, 17 * nx + ny + chain, chain=chain)
     assert info["passes"] >= 2
+    if nx in (1056, 20480, 528, 12288):          # windowed rows: passes of `chain` sub-steps
+        assert info["chain_x"] < n_steps or chain in (0, 24)
 
 
 @pytest.mark.parametrize("seg_rows", [16, 34, 64, 1024])
 @pytest.mark.parametrize("boundary", ["closed", "periodic"])
-def test_column_segments(seg_rows, boundary):
-    # segments shorter than the warm-up, ragged last segment, one segment for the whole column
-    cfg = G.make_cfg(192, 300, "f32", boundary, 0.3, 9)
-    check(cfg, 9, 5 + seg_rows, chain=8, seg_rows=seg_rows)
+@pytest.mark.parametrize("slots", [0, 2, 3, 5, 64])
+def test_column_segments_and_ring_depths(seg_rows, boundary, slots):
+    # segments shorter than the warm-up, ragged last segment, one segment for the whole column;
+    # any ring depth (clamped to [3, what shared memory holds]) gives the same result
+    if slots and seg_rows != 34:
+        pytest.skip("ring depths are swept at one segment size")
+    cfg = G.make_cfg(200, 300, "f32", boundary, 0.3, 9)
+    check(cfg, 9, 5 + seg_rows, chain=8, seg_rows=seg_rows, ring_slots=slots)
 
 
 @pytest.mark.parametrize("boundary", ["closed", "periodic"])
