@@ -6,7 +6,8 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline``
 
 The arithmetic lives in ``ts_oracle.c`` (plain C, double precision, the paper's operator
 sequence written out; citations there).  This file only builds it with gcc, loads it with
-ctypes and marshals numpy arrays.  ``window_evolve`` is the causal-window oracle of
+ctypes and marshals numpy arrays.  ``ts_oracle3d.c`` is the same statement for three-dimensional
+lattices (``sweep3``, ``evolve3``).  ``window_evolve`` is the causal-window oracle of
 SURVEY.md 8(c): the same C routine run on a cut-out whose margin exceeds the light cone
 (2 sites per step when the window origin is even), so it is exact on the interior.
 """
@@ -23,6 +24,9 @@ _HERE = Path(__file__).resolve().parent
 _SRC = _HERE / "ts_oracle.c"
 _LIB = _HERE / "libts_oracle.so"
 _lib = None
+_SRC3 = _HERE / "ts_oracle3d.c"
+_LIB3 = _HERE / "libts_oracle3d.so"
+_lib3 = None
 
 _D = ctypes.POINTER(ctypes.c_double)
 
@@ -35,6 +39,12 @@ def build(force: bool = False) -> Path:
                "-o", str(tmp), str(_SRC)]
         subprocess.run(cmd, check=True)
         os.replace(tmp, _LIB)
+    if force or not _LIB3.exists() or _LIB3.stat().st_mtime < _SRC3.stat().st_mtime:
+        tmp = _LIB3.with_suffix(f".so.tmp{os.getpid()}")
+        cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-Wall", "-Wextra",
+               "-o", str(tmp), str(_SRC3)]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB3)
     return _LIB
 
 
@@ -237,3 +247,70 @@ def window_evolve(fetch, nx: int, ny: int, x0: int, y0: int, w: int, h: int,
     evolve(re, im, a_half, b_half, a_full, b_full, pot=pot, periodic=False, n_steps=n_steps)
     ox, oy = x0 - lo_x, y0 - lo_y
     return re[oy:oy + h, ox:ox + w].copy(), im[oy:oy + h, ox:ox + w].copy()
+
+
+# ---- three-dimensional lattices (ts_oracle3d.c) ------------------------------
+
+def _load3():
+    global _lib3
+    if _lib3 is None:
+        build()
+        lib = ctypes.CDLL(str(_LIB3))
+        i64, dbl, i32 = ctypes.c_int64, ctypes.c_double, ctypes.c_int
+        _I = ctypes.POINTER(ctypes.c_int)
+        lib.oracle3_sweep.argtypes = [_D, _D, i64, i64, i64, i32, i32, dbl, dbl, i32]
+        lib.oracle3_sweep.restype = None
+        lib.oracle3_phase.argtypes = [_D, _D, i64, _D, _D]
+        lib.oracle3_phase.restype = None
+        lib.oracle3_evolve.argtypes = [_D, _D, i64, i64, i64, dbl, dbl, dbl, dbl, _D, _D, _I, i64]
+        lib.oracle3_evolve.restype = None
+        _lib3 = lib
+    return _lib3
+
+
+def _vol(a: np.ndarray) -> np.ndarray:
+    if a.dtype != np.float64 or a.ndim != 3 or not a.flags.c_contiguous or not a.flags.writeable:
+        raise ValueError("3-D oracle planes must be writable C-contiguous float64 [nz][ny][nx] arrays")
+    return a
+
+
+def _per3(periodic):
+    per = (periodic,) * 3 if isinstance(periodic, (bool, int, np.bool_)) else tuple(periodic)
+    if len(per) != 3:
+        raise ValueError("periodic: one flag or one per axis (x, y, z)")
+    return tuple(bool(p) for p in per)
+
+
+def sweep3(re, im, axis: int, parity: int, a: float, b: float, periodic: bool) -> None:
+    """In place: one checkerboard sweep of a [nz][ny][nx] lattice along axis 0 = x, 1 = y, 2 = z."""
+    _vol(re), _vol(im)
+    nz, ny, nx = re.shape
+    _load3().oracle3_sweep(_ptr(re), _ptr(im), nx, ny, nz, axis, parity, a, b, int(bool(periodic)))
+
+
+def evolve3(re, im, a_half, b_half, a_full, b_full, pot=None, periodic=False, n_steps=1) -> None:
+    """In place: n_steps second-order steps on a [nz][ny][nx] lattice.  periodic: one flag or
+    (px, py, pz); pot = None or (pot_re, pot_im) float64 arrays of the lattice's shape."""
+    _vol(re), _vol(im)
+    if im.shape != re.shape:
+        raise ValueError("re/im shape mismatch")
+    nz, ny, nx = re.shape
+    per = _per3(periodic)
+    for n, p in zip((nx, ny, nz), per):
+        if p and n % 2:
+            raise ValueError("a periodic axis needs an even extent")
+    pr = pi = None
+    if pot is not None:
+        pr = np.ascontiguousarray(pot[0], dtype=np.float64)
+        pi = np.ascontiguousarray(pot[1], dtype=np.float64)
+        assert pr.shape == re.shape and pi.shape == re.shape
+    flags = (ctypes.c_int * 3)(*[int(p) for p in per])
+    _load3().oracle3_evolve(_ptr(re), _ptr(im), nx, ny, nz, a_half, b_half, a_full, b_full,
+                            _ptr(pr), _ptr(pi), flags, int(n_steps))
+
+
+def norm2_3d(re, im) -> float:
+    """sum |psi|^2 of a 3-D state: the pinned 2-D routine on the same memory viewed as [nz*ny][nx]."""
+    re = np.ascontiguousarray(re, dtype=np.float64)
+    im = np.ascontiguousarray(im, dtype=np.float64)
+    return norm2(re.reshape(-1, re.shape[-1]), im.reshape(-1, im.shape[-1]))

@@ -337,9 +337,11 @@ def test_2048_default_options_full_lattice(recipe, opts):
     trap), 2048^2, 24 steps, every element against the full oracle."""
     cfg = inputs.scaled(inputs.CONFIGS[recipe], 2048, 2048, 24)
     (err, rel, drift, info), = _full_lattice_check(cfg, 24, [opts])
-    assert info["fused"] == 1 and info["seg_rows"] != 0
-    if recipe == "C4" and opts:
-        assert info["variant"] == 2
+    assert info["fused"] == 1
+    if recipe == "C4" and not opts:
+        assert info["variant"] == 4          # resident lines: one launch per axis, no segments
+    else:
+        assert info["variant"] == 2 and info["seg_rows"] != 0
     assert err <= G.tol(cfg), (err, info)
     assert rel <= (2e-5 if cfg.dtype == "f32" else 1e-11), (rel, info)
     assert abs(drift) < (1e-5 if cfg.dtype == "f32" else 1e-12)
