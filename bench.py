@@ -39,6 +39,23 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+# Plain-ALU peak: 148 SMs x 4 sub-partitions x 32 fp32 FMA lanes (16 fp64) x 2 flop at
+# the 1965 MHz maximum SM clock of the profiling guide -- derived, not measured.
+SM_COUNT, SM_MAX_MHZ = 148, 1965.0
+ALU_PEAK_TFLOPS = {"f32": SM_COUNT * 128 * 2 * SM_MAX_MHZ * 1e6 / 1e12,
+                   "f64": SM_COUNT * 64 * 2 * SM_MAX_MHZ * 1e6 / 1e12}
+
+
+def cpu_model():
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (profiling recipe line)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -85,37 +102,63 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_sample(cfg_name, budget_site_steps):
-    """(config, steps) of the bounded oracle sample: the workload's recipe on a smaller lattice."""
+def host_ram_bytes():
+    try:
+        for ln in open("/proc/meminfo"):
+            if ln.startswith("MemAvailable"):
+                return int(ln.split()[1]) * 1024
+    except OSError:
+        pass
+    return 0
+
+
+def oracle_sample(cfg_name, budget_site_steps, full_ok=False):
+    """(config, steps) of the bounded oracle sample: the workload's own lattice when the budget and
+    the host memory allow whole steps of it (C1-C3; C4: 2 steps of 16384^2, 4.3 GB of float64
+    state, only when full_ok), else the workload's recipe on a 2048^2 lattice (the cost is linear
+    in sites x steps)."""
     from paper_1208_2407_b200 import inputs
     cfg = inputs.CONFIGS[cfg_name]
+    need = cfg.sites * 8 * (2 + (2 if cfg.has_pot else 0)) * 2.5      # float64 planes + generation
+    ram = host_ram_bytes()
+    if cfg.sites <= budget_site_steps and (cfg.sites <= 2 ** 24 or (full_ok and need < 0.5 * ram)):
+        return cfg, max(1, min(cfg.n_steps, int(budget_site_steps // cfg.sites)))
     n = min(cfg.nx, 2048)
     small = inputs.scaled(cfg, n, n)
     steps = max(1, min(cfg.n_steps, int(budget_site_steps // small.sites)))
     return small, steps
 
 
-def time_oracle(cfg_name, budget_site_steps, repeats=1):
-    """Times oracle.evolve as it stands on all host cores; returns (rate, cores, sample text, s)."""
+def time_oracle(cfg_name, budget_site_steps, full_ok=False):
+    """Times oracle.evolve as it stands on ONE thread and on all host cores; returns a dict."""
     import numpy as np
     import oracle
     from paper_1208_2407_b200 import inputs
-    small, steps = oracle_sample(cfg_name, budget_site_steps)
+    small, steps = oracle_sample(cfg_name, budget_site_steps, full_ok)
     re, im, _ = inputs.full_state(small)
     pot = inputs.full_pot(small)
     re = re.astype(np.float64); im = im.astype(np.float64)
     potd = None if pot is None else (pot[0].astype(np.float64), pot[1].astype(np.float64))
-    oracle.evolve(re, im, *small.coeffs(), pot=potd, periodic=small.periodic, n_steps=1)  # warm
-    best = None
-    for _ in range(repeats):
-        t = time.perf_counter()
-        oracle.evolve(re, im, *small.coeffs(), pot=potd, periodic=small.periodic, n_steps=steps)
-        dt = time.perf_counter() - t
-        best = dt if best is None else min(best, dt)
-    rate = small.sites * steps / best
-    sample = (f"{small.nx}x{small.ny} sub-lattice of the {cfg_name} recipe ({small.boundary}, "
-              f"{'potential' if small.has_pot else 'no potential'}, float64), {steps} steps")
-    return rate, oracle.num_threads(), sample, best
+    c = small.coeffs()
+    cores = oracle.num_threads()
+    oracle.evolve(re, im, *c, pot=potd, periodic=small.periodic, n_steps=1)  # warm
+    t = time.perf_counter()
+    oracle.evolve(re, im, *c, pot=potd, periodic=small.periodic, n_steps=steps)
+    dt_all = time.perf_counter() - t
+    # one thread: a quarter of the steps (at least one), same lattice
+    steps1 = max(1, steps // 4) if cores > 1 else steps
+    oracle.set_num_threads(1)
+    t = time.perf_counter()
+    oracle.evolve(re, im, *c, pot=potd, periodic=small.periodic, n_steps=steps1)
+    dt_one = time.perf_counter() - t
+    oracle.set_num_threads(cores)
+    sample = (f"{small.nx}x{small.ny} {'(the full lattice)' if small.nx == inputs.CONFIGS[cfg_name].nx else 'sub-lattice'}"
+              f" of the {cfg_name} recipe ({small.boundary}, "
+              f"{'potential' if small.has_pot else 'no potential'}, float64), {steps} steps on "
+              f"{cores} threads, {steps1} on one")
+    return {"value": small.sites * steps / dt_all, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": sample, "seconds": dt_all, "value_1thread": small.sites * steps1 / dt_one,
+            "nproc": os.cpu_count(), "cpu_model": cpu_model()}
 
 
 def run_reference(args):
@@ -149,12 +192,104 @@ def run_reference(args):
         "data": "synthetic",
         "config": {"workload": workload_text(cfg), "sample": sample},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(),
-                         "kind": "oracle", "sample": sample},
+                         "kind": "oracle", "sample": sample, "nproc": os.cpu_count(),
+                         "cpu_model": cpu_model()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
     return 0
+
+
+def work_of(kind, cfg, sep, info, eb):
+    """Algorithmic (bytes, flops) of ONE launch of a kernel kind.
+    Bytes: every plane the launch must read and write once.  Flops: 2 FMAs = 4 flops per site and
+    pair sweep in the scaled form; without a potential a sub-step is 2 sweeps per axis (adjacent
+    half sweeps merged), with one it is 7 sweeps + the phase (2 FMA + 2 MUL) = 34 flops."""
+    sites = cfg.sites
+    state = 4 * eb * sites                       # read + write of both planes
+    S = max(1, info["fuse_steps"])
+    if kind in (2, 3):                           # fused / stream pass: S whole sub-steps
+        planes = cfg.has_pot and not sep
+        by = state + (2 * eb * sites if planes else 0)
+        fl = sites * S * (34 if cfg.has_pot else 16)
+        return by, fl
+    if kind in (5, 6, 11):                       # resident lines: all sub-steps of one axis
+        return state, sites * cfg.n_steps * 8
+    if kind == 7:
+        return state, sites * max(1, info["chain_x"]) * 8
+    if kind == 8:
+        return state, sites * max(1, info["chain_y"]) * 8
+    if kind == 9:
+        return state, 0
+    if kind == 4:                                # whole evolution on chip
+        return state, sites * cfg.n_steps * (34 if cfg.has_pot else 16)
+    if kind == 1:                                # per-sweep kernels of the whole call
+        sweeps = 9 if cfg.has_pot else 7
+        return state * sweeps * cfg.n_steps, sites * cfg.n_steps * (34 if cfg.has_pot else 28)
+    return state, 0
+
+
+def roofline_of(cfg, sep, info, per_kind, calls, hbm_peak, peak_src, call_ms):
+    """The roofline object of the bench line: the kernel kind with the largest share of the call,
+    its own average event time, and whichever of HBM and plain ALU binds it."""
+    from paper_1208_2407_b200.binding import LAUNCH_KINDS
+    eb = 4 if cfg.dtype == "f32" else 8
+    alu_peak = ALU_PEAK_TFLOPS[cfg.dtype]
+    if not per_kind:
+        return {"bound": "hbm", "achieved": None, "peak": hbm_peak, "unit": "GB/s", "frac": None,
+                "traffic": None, "note": "no launch times recorded"}
+    shares = {k: sum(v) / calls for k, v in per_kind.items()}
+    total = sum(shares.values())
+    floor_ms = 0.0
+    kernels = []
+    for k, v in sorted(per_kind.items(), key=lambda kv: -sum(kv[1])):
+        by, fl = work_of(k, cfg, sep, info, eb)
+        avg = sum(v) / len(v)
+        t_hbm = by / (hbm_peak * 1e9) * 1e3
+        t_alu = fl / (alu_peak * 1e12) * 1e3
+        floor_ms += max(t_hbm, t_alu) * len(v) / calls
+        kernels.append({"kernel": LAUNCH_KINDS.get(k, str(k)), "launches_per_call": len(v) // calls,
+                        "avg_ms": avg, "share": shares[k] / total,
+                        "hbm_frac": t_hbm / avg, "alu_frac": t_alu / avg,
+                        "GB/s": by / avg / 1e6, "TFLOP/s": fl / avg / 1e9})
+    top = kernels[0]
+    kind = max(shares, key=shares.get)
+    by, fl = work_of(kind, cfg, sep, info, eb)
+    bound = "alu" if top["alu_frac"] > top["hbm_frac"] else "hbm"
+    traffic = tsrc = None
+    tp = ROOT / "profiles" / "traffic.json"
+    key = f"{cfg.name}:{top['kernel']}"
+    if tp.exists():
+        try:
+            traffic = json.loads(tp.read_text()).get(key)
+            tsrc = f"profiles/traffic.json[{key}]: one ncu --set full capture of this kernel, not this run"
+        except (ValueError, OSError):
+            traffic = None
+    chain = {5: cfg.n_steps, 6: cfg.n_steps, 7: info["chain_x"], 8: info["chain_y"]}.get(
+        kind, max(1, info["fuse_steps"]))
+    roof = {
+        "bound": bound,
+        "achieved": top["TFLOP/s"] if bound == "alu" else top["GB/s"],
+        "peak": alu_peak if bound == "alu" else hbm_peak,
+        "unit": "TFLOP/s" if bound == "alu" else "GB/s",
+        "frac": top["alu_frac"] if bound == "alu" else top["hbm_frac"],
+        "traffic": traffic, "traffic_source": tsrc,
+        "kernel": f"{top['kernel']}<{cfg.dtype}>, {chain} sub-steps per launch",
+        "launch_ms": top["avg_ms"], "launches_per_call": top["launches_per_call"],
+        "share_of_call": top["share"],
+        "bytes_per_launch": by, "flops_per_launch": fl,
+        "peak_source": (f"HBM: {peak_src}; ALU: derived, {SM_COUNT} SMs x "
+                        f"{128 if cfg.dtype == 'f32' else 64} FMA lanes x 2 x {SM_MAX_MHZ:.0f} MHz"),
+        "hbm": {"achieved": top["GB/s"], "peak": hbm_peak, "frac": top["hbm_frac"],
+                "frac_of_8TBs_nominal": top["GB/s"] / 8000.0},
+        "alu": {"achieved": top["TFLOP/s"], "peak": alu_peak, "frac": top["alu_frac"]},
+        "kernels": kernels,
+        # the whole call against the sum over its launches of max(HBM time, ALU time)
+        "call": {"event_ms_sum": total, "call_ms": call_ms, "roofline_ms": floor_ms,
+                 "frac": floor_ms / call_ms},
+    }
+    return roof
 
 
 def workload_text(cfg):
@@ -196,6 +331,10 @@ def run_gpu(args):
         plan.set_option("fuse_steps", args.fuse_steps)
     if args.seg_rows:
         plan.set_option("seg_rows", args.seg_rows)
+    if args.chain:
+        plan.set_option("chain", args.chain)
+    if args.variant:
+        plan.set_option("variant", args.variant)
     c = cfg.coeffs()
     stream = torch.cuda.current_stream()
 
@@ -235,8 +374,21 @@ def run_gpu(args):
         ms = float(t.item())
     n1 = plan.norm(re, im)
     info = {k: plan.info(k) for k in ("fused", "fuse_steps", "passes", "launches", "seg_rows",
-                                     "variant")}
+                                     "variant", "chain_x", "chain_y")}
     value = world * cfg.sites * cfg.n_steps * args.steps / (ms * 1e-3)
+
+    # per-kernel device times of the same call: the library brackets every launch with CUDA events
+    # on the launch stream (plan option "timing"); a few calls right after the timed region,
+    # same clocks and thermal state.  The timed region above runs without them.
+    plan.set_option("timing", 1)
+    per_kind = {}
+    timing_calls = max(1, min(args.steps, 3))
+    for _ in range(timing_calls):
+        evolve_once()
+        torch.cuda.synchronize()
+        for kind, kms in plan.launch_times():
+            per_kind.setdefault(kind, []).append(kms)
+    plan.set_option("timing", 0)
 
     # end to end through ts_evolve_host: pinned host planes, H2D + D2H inside the timed region
     hre = torch.empty((cfg.ny, cfg.nx), dtype=tdt, pin_memory=True)
@@ -285,44 +437,32 @@ def run_gpu(args):
     peak, peak_src = load_peaks()
     S = max(1, info["fuse_steps"])
     passes = max(1, info["passes"])
-    # algorithmic bytes of one fused launch: read + write both planes once (+ phase planes once)
-    bytes_per_launch = cfg.sites * (4 * eb + (2 * eb if (cfg.has_pot and sep is None) else 0))
-    launch_ms = ms / (args.steps * passes)
-    achieved = bytes_per_launch / (launch_ms * 1e-3) / 1e9
-    traffic = None
-    tp = ROOT / "profiles" / "traffic.json"
-    if tp.exists():
-        try:
-            traffic = json.loads(tp.read_text()).get(f"{cfg.name}_S{S}")
-        except (ValueError, OSError):
-            traffic = None
-    cpu_rate, cores, sample, cpu_s = time_oracle(args.config, args.cpu_budget)
+    roof = roofline_of(cfg, sep is not None, info, per_kind, timing_calls, peak, peak_src,
+                       ms / args.steps)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
         "config": {"workload": workload_text(cfg) + (" (separable factors, ts_evolve_sep)"
                                                      if sep is not None else ""),
+                   "variant": {0: "per-sweep kernels", 1: "fused_kernel", 2: "stream_kernel",
+                               3: "tiny_kernel", 4: "axis-split"}.get(info["variant"]),
                    "fuse_steps": S, "passes_per_call": passes,
+                   "chain_x": info["chain_x"], "chain_y": info["chain_y"],
                    "seg_rows": info["seg_rows"], "fused": info["fused"],
                    "parallelism": "replicas only (no sharding of one lattice)",
-                   "l2": "state (2 planes x 2 buffers) far larger than the 126 MB L2; no flush",
+                   "l2": ("state (2 planes x 2 buffers) far larger than the 126 MB L2; no flush"
+                          if cfg.sites * eb * 4 > 2 * 126e6 else
+                          "state fits the 126 MB L2 (the workload IS the L2-resident case; no flush)"),
                    "norm2_before": n0, "norm_drift": n1 / n0 - 1},
         "clocks": clocks,
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3,
-                "api": e2e_api},
+                "api": e2e_api,
+                "note": "host<->device copies and compute are serialised inside the call"},
         "gpu_launches": info["launches"] * args.steps,
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": traffic,
-                     "kernel": f"{'stream_kernel' if info['variant'] == 2 else 'fused_kernel'}"
-                               f"<{cfg.dtype}, S={S}>",
-                     "bytes_per_launch": bytes_per_launch, "launch_ms": launch_ms,
-                     "peak_source": peak_src,
-                     "site_step_roofline": peak * 1e9 / (bytes_per_launch / cfg.sites / S),
-                     "frac_of_8TBs_nominal": achieved / 8000.0},
-        "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-                         "sample": sample, "seconds": cpu_s},
+        "roofline": roof,
+        "cpu_baseline": time_oracle(args.config, args.cpu_budget, full_ok=True),
     }
     print(json.dumps(line), flush=True)
     if dist is not None:
@@ -477,6 +617,8 @@ def main():
     ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--fuse-steps", type=int, default=0)
     ap.add_argument("--seg-rows", type=int, default=0)
+    ap.add_argument("--chain", type=int, default=0, help="axis-split path: sub-steps per pass")
+    ap.add_argument("--variant", type=int, default=0, help="plan option variant (0 = default path)")
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: independent lattices per GPU (default, north_star) or one lattice "
                          "cut into row slabs with NCCL halo exchange")

@@ -1,6 +1,7 @@
 /*
- * ts.h -- C ABI of libts: second-order Trotter-Suzuki time step for one particle on a 2-D
- * lattice, NVIDIA B200 (sm_100a).  Plain pointers and sizes only; no C++/torch types.
+ * ts.h -- C ABI of libts: second-order Trotter-Suzuki time step for one particle on a 2-D (or 3-D:
+ * ts_plan_create_3d) lattice, NVIDIA B200 (sm_100a).  Plain pointers and sizes only; no C++/torch
+ * types.
  *
  * What it computes (PAPER.md = the paper's text; readings R1..R13 are listed in DESIGN.md):
  *   The lattice Hamiltonian is split into a diagonal part H0 and, per axis, an even-pair and an
@@ -57,9 +58,39 @@ ts_plan* ts_plan_create(int64_t nx, int64_t ny, int dtype, int boundary);
  * a row slab of a larger periodic lattice needs (domain decomposition: the
  * slab plus its halo rows is evolved as a lattice that is closed in y; the rows within 2 sites per
  * step of a cut are then wrong and are the halo that the next exchange overwrites).
- * (TS_CLOSED, TS_PERIODIC) runs on the per-sweep kernels only.
+ * (TS_CLOSED, TS_PERIODIC) with a potential runs on the per-sweep kernels only.
  */
 ts_plan* ts_plan_create_xy(int64_t nx, int64_t ny, int dtype, int boundary_x, int boundary_y);
+
+/*
+ * ts_plan_create_3d -- a THREE-dimensional lattice nx x ny x nz, the extension the paper names as its
+ * next direction along the lines it gives for more than one dimension ("the
+ * diagonal energies, and two terms for each dimension").  One boundary type per
+ * axis, as for ts_plan_create_xy; a periodic axis needs an even extent.  Layout: planes
+ * psi[nz][ny][nx], x fastest, element (x, y, z) at (z*ny + y)*nx + x.  Such a plan is evolved with
+ * ts_evolve_3d only (ts_norm works on it; the 2-D entry points return TS_EINVAL).
+ */
+ts_plan* ts_plan_create_3d(int64_t nx, int64_t ny, int64_t nz, int dtype,
+                           int boundary_x, int boundary_y, int boundary_z);
+
+/*
+ * ts_evolve_3d -- psi <- U2^n_steps psi on a plan from ts_plan_create_3d, in place, with the step
+ *
+ *      Xe(h) Xo(h) Ye(h) Yo(h) Ze(h) [ Zo(f) | Zo(h) P Zo(h) ] Ze(h) Yo(h) Ye(h) Xo(h) Xe(h)
+ *
+ * (Eq. 3 with seven parts; reading R14: the 2-D order with the new axis innermost).
+ * Arguments as for ts_evolve; pot_phase_or_null is 2*nz*ny*nx elements (Re plane, then Im plane).
+ * Paths: sweeps along different axes commute, so without a potential the n_steps steps are three
+ * chains (one launch per axis, every line resident in registers for all steps), and with one the
+ * sweeps between two applications of the phase regroup per axis into O(h) E(2h) O(h): three
+ * launches per step.  Both need even extents of at most 16384 (fp32) / 8192 (fp64) sites per axis
+ * in a shape a thread block holds, and cos of every sweep angle > 0.25; other lattices run on the
+ * per-sweep kernels (11 / 13 launches per step).  Option "path" = 1 forces those, "path" = 2 or
+ * "variant" = 4 requires the fused path (TS_EUNSUPPORTED otherwise).  No scratch is used.
+ */
+int ts_evolve_3d(ts_plan* plan, void* psi_re, void* psi_im,
+                 double a_half, double b_half, double a_full, double b_full,
+                 const void* pot_phase_or_null, int64_t n_steps, void* cuda_stream);
 
 /*
  * ts_evolve -- psi <- U2^n_steps psi, in place from the caller's view (Eq. 3).
@@ -188,20 +219,55 @@ int ts_evolve_host(ts_plan* plan, void* psi_re_host, void* psi_im_host,
  *                  planes on the TMA ring kernel), 0 = auto.
  *   "seg_rows"     rows of output per streaming segment of the fused kernel (even), 0 = auto;
  *                  for the on-chip kernel (variant 3): rows per warp, 2 / 4 / 8, 0 = auto.
- *   "variant"      0 = auto, 1 = register-prefetch kernel, 2 = TMA ring kernel (the default
- *                  wherever it applies: nx >= 128 or closed in x), 3 = on-chip-resident kernel:
- *                  the whole lattice in the registers of one thread block and all n_steps in
- *                  one launch (the default for uniform steps on lattices up to 128 x 128 sites in
- *                  fp32, 128 x 64 in fp64, half that with a potential).
+ *   "variant"      0 = auto, 1 = register-prefetch kernel, 2 = TMA ring kernel (the default with a
+ *                  potential wherever it applies: nx >= 128 or closed in x), 3 = on-chip-resident
+ *                  kernel: the whole lattice in the registers of one thread block and all n_steps
+ *                  in one launch (lattices up to 128 x 128 sites in fp32, 128 x 64 in fp64, half
+ *                  that with a potential; the default there WITH a potential), 4 = axis-split path
+ *                  (the default WITHOUT a potential, nx % 4 == 0, even ny): the step then
+ *                  factorises exactly into a chain of sweeps along every row times a chain along
+ *                  every column (X and Y sweeps commute); lines that fit a thread
+ *                  block stay in registers for ALL n_steps (one launch per axis), longer rows are
+ *                  cut into windows with a halo, longer columns stream through a register pipeline.
+ *   "chain"        axis-split path: sub-steps per windowed / pipelined pass (<= 24 fp32, 12 fp64),
+ *                  0 = auto.
  *   "ring_slots"   row-pair slots of the TMA ring per warp, 0 = auto.
+ *   "timing"       1: record CUDA events around every launch (ts_plan_get_launch_times), 0 = off.
  * Environment: TS_NO_PDL=1 turns off programmatic dependent launch between passes.
  */
 int ts_plan_set_option(ts_plan* plan, const char* name, int64_t value);
 
 /* ts_plan_get_info -- read back what the last ts_evolve* / ts_slab_pass used:
  *   "fused" (0/1), "fuse_steps", "passes", "launches" (kernels + copies enqueued), "seg_rows",
- *   "variant" (1 / 2 / 3, 0 on the per-sweep path). */
+ *   "variant" (1 / 2 / 3 / 4, 0 on the per-sweep path), "chain_x", "chain_y" (axis-split path:
+ *   sub-steps per launch along the rows / the columns). */
 int ts_plan_get_info(const ts_plan* plan, const char* name, int64_t* out_value);
+
+/*
+ * ts_plan_reserve -- allocate now what ts_evolve* would allocate on first use (the second state
+ * buffer for the double-buffered passes, and the reduction workspace of ts_norm), so
+ * that no later call contains a device allocation.  with_host_staging != 0 also reserves the
+ * device staging buffers of ts_evolve_host (state; plus phase planes if with_host_staging == 2).
+ * Errors: TS_EINVAL (NULL plan, other device current), TS_EALLOC.
+ */
+int ts_plan_reserve(ts_plan* plan, int with_host_staging);
+
+/*
+ * ts_plan_get_launch_times -- device time of every launch of the LAST ts_evolve* call on this plan,
+ * measured by CUDA events that the library records on the launch stream around each kernel (and
+ * around the final plane copies) when the plan option "timing" is 1.  bench.py reports its
+ * roofline from these (the dominant kernel's own time, not the call divided by the launch count).
+ *   max_n      capacity of the two output arrays.
+ *   kinds_out  HOST array: what was launched -- 1 per-sweep kernels of one whole call, 2 fused_kernel
+ *              pass, 3 stream_kernel pass, 4 tiny_kernel, 5 line_kernel along rows, 6 line_kernel
+ *              along columns, 7 xwin_kernel pass, 8 ycol_kernel pass, 9 plane copies, 10 separable
+ *              phase expansion, 11 line_kernel along z, 12 phase kernel (3-D).
+ *   ms_out     HOST array: milliseconds.
+ *   n_out      HOST int: number of launches recorded (may exceed max_n; then only max_n are written).
+ * Synchronises with the recorded events.  With "timing" 0 (the default) nothing is recorded and
+ * *n_out is 0.  Errors: TS_EINVAL, TS_ECUDA.
+ */
+int ts_plan_get_launch_times(ts_plan* plan, int max_n, int* kinds_out, float* ms_out, int* n_out);
 
 int ts_plan_destroy(ts_plan* plan);           /* NULL is accepted (no-op, TS_OK) */
 

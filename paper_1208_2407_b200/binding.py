@@ -13,9 +13,16 @@ TS_MAX_FUSE = 6
 _LIB_PATH = Path(__file__).resolve().parent / "libts.so"
 _lib = None
 
-SYMBOLS = ["ts_plan_create", "ts_plan_create_xy", "ts_evolve", "ts_evolve_u4", "ts_evolve_sep", "ts_evolve_tdep", "ts_slab_pass",
+SYMBOLS = ["ts_plan_create", "ts_plan_create_xy", "ts_plan_create_3d", "ts_evolve", "ts_evolve_3d", "ts_evolve_u4", "ts_evolve_sep", "ts_evolve_tdep", "ts_slab_pass",
            "ts_norm", "ts_evolve_host", "ts_plan_set_option",
-           "ts_plan_get_info", "ts_plan_destroy", "ts_last_error"]
+           "ts_plan_get_info", "ts_plan_reserve", "ts_plan_get_launch_times", "ts_plan_destroy",
+           "ts_last_error"]
+
+# kinds reported by ts_plan_get_launch_times (include/ts.h)
+LAUNCH_KINDS = {1: "per-sweep kernels", 2: "fused_kernel", 3: "stream_kernel", 4: "tiny_kernel",
+                5: "line_kernel(rows)", 6: "line_kernel(columns)", 7: "xwin_kernel",
+                8: "ycol_kernel", 9: "plane copies", 10: "expand_separable", 11: "line_kernel(z)",
+                12: "phase_kernel"}
 
 
 class TsError(RuntimeError):
@@ -37,8 +44,12 @@ def lib():
         L.ts_plan_create.restype = vp
         L.ts_plan_create_xy.argtypes = [i64, i64, i32, i32, i32]
         L.ts_plan_create_xy.restype = vp
+        L.ts_plan_create_3d.argtypes = [i64, i64, i64, i32, i32, i32, i32]
+        L.ts_plan_create_3d.restype = vp
         L.ts_evolve.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp, i64, vp]
         L.ts_evolve.restype = i32
+        L.ts_evolve_3d.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp, i64, vp]
+        L.ts_evolve_3d.restype = i32
         L.ts_evolve_u4.argtypes = [vp, vp, vp, dbl, vp, vp, i64, vp]
         L.ts_evolve_u4.restype = i32
         L.ts_evolve_sep.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp, vp, i64, vp]
@@ -56,6 +67,11 @@ def lib():
         L.ts_plan_set_option.restype = i32
         L.ts_plan_get_info.argtypes = [vp, ctypes.c_char_p, ctypes.POINTER(i64)]
         L.ts_plan_get_info.restype = i32
+        L.ts_plan_reserve.argtypes = [vp, i32]
+        L.ts_plan_reserve.restype = i32
+        L.ts_plan_get_launch_times.argtypes = [vp, i32, ctypes.POINTER(i32),
+                                               ctypes.POINTER(ctypes.c_float), ctypes.POINTER(i32)]
+        L.ts_plan_get_launch_times.restype = i32
         L.ts_plan_destroy.argtypes = [vp]
         L.ts_plan_destroy.restype = i32
         L.ts_last_error.argtypes = []
@@ -113,6 +129,20 @@ class Plan:
         out = ctypes.c_int64(0)
         _check(lib().ts_plan_get_info(self._h, name.encode(), ctypes.byref(out)))
         return out.value
+
+    def reserve(self, with_host_staging: int = 0):
+        _check(lib().ts_plan_reserve(self._h, int(with_host_staging)))
+
+    def launch_times(self):
+        """[(kind, ms), ...] of the last evolve call (plan option "timing" = 1)."""
+        n = ctypes.c_int(0)
+        _check(lib().ts_plan_get_launch_times(self._h, 0, None, None, ctypes.byref(n)))
+        if n.value == 0:
+            return []
+        kinds = (ctypes.c_int * n.value)()
+        ms = (ctypes.c_float * n.value)()
+        _check(lib().ts_plan_get_launch_times(self._h, n.value, kinds, ms, ctypes.byref(n)))
+        return [(int(kinds[i]), float(ms[i])) for i in range(n.value)]
 
     def _planes(self, re, im):
         if re.dtype != self.dtype or im.dtype != self.dtype:
@@ -253,3 +283,43 @@ class Plan:
             self.destroy()
         except Exception:
             pass
+
+
+class Plan3D(Plan):
+    """ts_plan_create_3d: a lattice nx x ny x nz, planes [nz][ny][nx] (x fastest).  boundary: one
+    name or a tuple (x, y, z) of "closed" / "periodic".  evolve = ts_evolve_3d; norm = ts_norm."""
+
+    def __init__(self, nx: int, ny: int, nz: int, dtype, boundary="closed"):
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.dtype = dtype
+        codes = {"closed": TS_CLOSED, "periodic": TS_PERIODIC}
+        b = (boundary,) * 3 if isinstance(boundary, str) else tuple(boundary)
+        self._h = lib().ts_plan_create_3d(self.nx, self.ny, self.nz, _dtype_code(dtype),
+                                          codes[b[0]], codes[b[1]], codes[b[2]])
+        if not self._h:
+            raise TsError(TS_EINVAL, last_error())
+
+    def _planes(self, re, im):
+        if re.dtype != self.dtype or im.dtype != self.dtype:
+            raise TypeError("plane dtype differs from the plan's")
+        shape = (self.nz, self.ny, self.nx)
+        if tuple(re.shape) != shape or tuple(im.shape) != shape:
+            raise ValueError(f"planes must have shape [nz][ny][nx] = {shape}")
+        if not (re.is_contiguous() and im.is_contiguous()):
+            raise ValueError("planes must be contiguous")
+
+    def evolve(self, psi_re, psi_im, a_half, b_half, a_full, b_full, pot_phase=None,
+               n_steps=1, stream=None):
+        """ts_evolve_3d on CUDA tensors, in place, asynchronous on `stream` (default: current)."""
+        self._planes(psi_re, psi_im)
+        if not (psi_re.is_cuda and psi_im.is_cuda):
+            raise ValueError("evolve takes CUDA tensors")
+        pot = None
+        if pot_phase is not None:
+            if pot_phase.dtype != self.dtype or not pot_phase.is_contiguous() or not pot_phase.is_cuda \
+                    or tuple(pot_phase.shape) != (2, self.nz, self.ny, self.nx):
+                raise ValueError("pot_phase must be a contiguous CUDA tensor [2][nz][ny][nx]")
+            pot = ctypes.c_void_p(pot_phase.data_ptr())
+        _check(lib().ts_evolve_3d(self._h, ctypes.c_void_p(psi_re.data_ptr()),
+                                  ctypes.c_void_p(psi_im.data_ptr()), a_half, b_half, a_full,
+                                  b_full, pot, int(n_steps), _stream_handle(stream)))

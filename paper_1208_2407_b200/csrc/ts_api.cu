@@ -18,10 +18,31 @@ int cuda_fail(cudaError_t e, const char* what) {
     return TS_ECUDA;
 }
 
+void LaunchTimer::begin(int kind, cudaStream_t st) {
+    if (used == recs.size()) {
+        Rec r{kind, nullptr, nullptr};
+        if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) {
+            (void)cudaGetLastError();
+            return;
+        }
+        recs.push_back(r);
+    }
+    recs[used].kind = kind;
+    cudaEventRecord(recs[used].a, st);
+}
+void LaunchTimer::end(cudaStream_t st) {
+    if (used < recs.size()) cudaEventRecord(recs[used++].b, st);
+}
+LaunchTimer::~LaunchTimer() {
+    for (Rec& r : recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+}
+
 }  // namespace ts
 
 struct ts_plan {
     ts::LatticeDesc L;
+    int64_t nz;               // 1: two-dimensional plan; else psi[nz][ny][nx] (ts_plan_create_3d)
+    int periodic_z;
     int device;
     size_t elem;              // bytes per element
     // scratch state buffer for the double-buffered fused passes
@@ -40,6 +61,8 @@ struct ts_plan {
     // info on the last ts_evolve
     int64_t info_fused, info_fuse, info_passes, info_launches, info_seg, info_variant;
     int64_t info_chain_x, info_chain_y;
+    int64_t opt_timing;
+    ts::LaunchTimer* timer;   // allocated when option "timing" is first set
 };
 
 namespace {
@@ -115,8 +138,34 @@ ts_plan* ts_plan_create_xy(int64_t nx, int64_t ny, int dtype, int boundary, int 
     if (!p) { set_error("out of host memory"); return nullptr; }
     memset(p, 0, sizeof(*p));
     p->L.nx = nx; p->L.ny = ny; p->L.dtype = dtype; p->L.periodic_x = boundary == TS_PERIODIC; p->L.periodic_y = boundary_y == TS_PERIODIC;
+    p->nz = 1;
     p->device = dev;
     p->elem = dtype == TS_F32 ? 4 : 8;
+    return p;
+}
+
+ts_plan* ts_plan_create_3d(int64_t nx, int64_t ny, int64_t nz, int dtype, int boundary_x,
+                           int boundary_y, int boundary_z) {
+    if (nz < 1) { set_error("nz must be >= 1"); return nullptr; }
+    if (boundary_z != TS_CLOSED && boundary_z != TS_PERIODIC) {
+        set_error("unknown boundary");
+        return nullptr;
+    }
+    if (boundary_z == TS_PERIODIC && nz % 2) {
+        set_error("a periodic axis needs an even extent (an odd ring cannot be split into "
+                  "disjoint pairs)");
+        return nullptr;
+    }
+    if (nx < 1 || ny < 1 || nx > (int64_t(1) << 31) || ny > (int64_t(1) << 31) ||
+        nz > (int64_t(1) << 31) ||
+        (double)nx * (double)ny * (double)nz >= (double)((int64_t(1) << 62) / 16)) {
+        set_error("lattice too large");
+        return nullptr;
+    }
+    ts_plan* p = ts_plan_create_xy(nx, ny, dtype, boundary_x, boundary_y);
+    if (!p) return nullptr;
+    p->nz = nz;
+    p->periodic_z = boundary_z == TS_PERIODIC;
     return p;
 }
 
@@ -130,6 +179,7 @@ int ts_plan_destroy(ts_plan* plan) {
     cudaFree(plan->host_pot);
     cudaFree(plan->sep_pot);
     if (plan->own_stream) cudaStreamDestroy(plan->own_stream);
+    delete plan->timer;
     delete plan;
     return TS_OK;
 }
@@ -151,6 +201,13 @@ int ts_plan_set_option(ts_plan* plan, const char* name, int64_t value) {
     } else if (!strcmp(name, "chain")) {
         if (value < 0 || value > 64) return fail(TS_EINVAL, "chain out of range");
         plan->opt_chain = value;
+    } else if (!strcmp(name, "timing")) {
+        if (value != 0 && value != 1) return fail(TS_EINVAL, "timing must be 0 or 1");
+        if (value && !plan->timer) {
+            plan->timer = new (std::nothrow) ts::LaunchTimer();
+            if (!plan->timer) return fail(TS_EALLOC, "out of host memory");
+        }
+        plan->opt_timing = value;
     } else if (!strcmp(name, "ring_slots")) {
         if (value < 0 || value > 64) return fail(TS_EINVAL, "ring_slots out of range");
         plan->opt_slots = value;
@@ -193,6 +250,7 @@ bool same_phase(const ts::Phase& a, const ts::Phase& b) {
 int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat, int period,
                    int64_t n_repeat, void* cuda_stream) {
     if (!plan) return fail(TS_EINVAL, "NULL plan");
+    if (plan->nz != 1) return fail(TS_EINVAL, "three-dimensional plan: use ts_evolve_3d");
     if (!psi_re || !psi_im) return fail(TS_EINVAL, "NULL psi plane");
     if (n_repeat < 0) return fail(TS_EINVAL, "n_steps < 0");
     const ts::LatticeDesc& L = plan->L;
@@ -241,6 +299,8 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
     int rc = check_device(plan);
     if (rc != TS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    ts::LaunchTimer* tm = plan->opt_timing ? plan->timer : nullptr;
+    if (plan->timer) plan->timer->reset();
 
     plan->info_fused = plan->info_fuse = plan->info_passes = plan->info_launches = 0;
     plan->info_seg = plan->info_variant = plan->info_chain_x = plan->info_chain_y = 0;
@@ -298,7 +358,7 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
         ts::AxisInfo ai;
         rc = ts::axis_evolve(L, psi_re, psi_im, plan->scratch_re, plan->scratch_im, axis_pat, period,
                              n_sub, (int)plan->opt_chain, (int)plan->opt_seg, (int)plan->opt_slots,
-                             st, &ai);
+                             st, &ai, tm);
         plan->info_launches = ai.launches;
         if (rc != TS_OK) return rc;
         plan->info_fused = 1; plan->info_passes = ai.passes; plan->info_seg = ai.seg_rows;
@@ -307,8 +367,10 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
         return TS_OK;
     }
     if (use_tiny) {
+        ts::timer_begin(tm, ts::kKindTiny, st);
         rc = ts::tiny_evolve(L, psi_re, psi_im, pat[0].c, pat[0].ph.planes, n_repeat,
                              (int)plan->opt_seg, st);     // "seg_rows" = rows per warp here
+        ts::timer_end(tm, st);
         if (rc != TS_OK) return rc;
         plan->info_fused = 1; plan->info_fuse = n_repeat; plan->info_passes = 1;
         plan->info_launches = 1; plan->info_seg = L.ny; plan->info_variant = 3;
@@ -320,7 +382,9 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
     if (expand_sep) {
         rc = ensure_alloc(&plan->sep_pot, 2 * plane_bytes);
         if (rc != TS_OK) return rc;
+        ts::timer_begin(tm, ts::kKindExpand, st);
         rc = ts::expand_separable(L, pat[0].ph.px, pat[0].ph.py, plan->sep_pot, st);
+        ts::timer_end(tm, st);
         if (rc != TS_OK) return rc;
         ++plan->info_launches;
         expanded = pat[0];
@@ -330,8 +394,10 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
     if (generic) {
         const int64_t l0 = plan->info_launches;
         if (period == 1) {
+            ts::timer_begin(tm, ts::kKindGeneric, st);
             rc = ts::generic_evolve(L, psi_re, psi_im, pat[0].c, pat[0].ph.planes, n_repeat, st,
                                     &plan->info_launches);
+            ts::timer_end(tm, st);
             plan->info_launches += l0;
             return rc;
         }
@@ -370,11 +436,13 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
             if (!use_stream && s > 0 && memcmp(&x.c, &subs[0], sizeof(ts::StepCoef)) != 0) break;
             subs[s++] = x.c;
         }
+        ts::timer_begin(tm, use_stream ? ts::kKindStream : ts::kKindFused, st);
         if (use_stream)
             rc = ts::stream_pass(L, cur_re, cur_im, nxt_re, nxt_im, subs, ph, s, seg,
                                  (int)plan->opt_slots, st);
         else
             rc = ts::fused_pass(L, cur_re, cur_im, nxt_re, nxt_im, subs[0], ph.planes, s, seg, st);
+        ts::timer_end(tm, st);
         if (rc != TS_OK) return rc;
         void* t;
         t = cur_re; cur_re = nxt_re; nxt_re = t;
@@ -384,8 +452,10 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
         ++plan->info_launches;
     }
     if (cur_re != psi_re) {   // odd number of passes: the result sits in the scratch buffer
+        ts::timer_begin(tm, ts::kKindCopy, st);
         TS_CUDA_TRY(cudaMemcpyAsync(psi_re, cur_re, plane_bytes, cudaMemcpyDeviceToDevice, st));
         TS_CUDA_TRY(cudaMemcpyAsync(psi_im, cur_im, plane_bytes, cudaMemcpyDeviceToDevice, st));
+        ts::timer_end(tm, st);
         plan->info_launches += 2;
     }
     plan->info_fused = 1;
@@ -405,6 +475,55 @@ int ts_evolve(ts_plan* plan, void* psi_re, void* psi_im, double a_half, double b
     return evolve_pattern(plan, psi_re, psi_im, &one, 1, n_steps, cuda_stream);
 }
 
+int ts_evolve_3d(ts_plan* plan, void* psi_re, void* psi_im, double a_half, double b_half,
+                 double a_full, double b_full, const void* pot, int64_t n_steps, void* cuda_stream) {
+    if (!plan) return fail(TS_EINVAL, "NULL plan");
+    if (!psi_re || !psi_im) return fail(TS_EINVAL, "NULL psi plane");
+    if (n_steps < 0) return fail(TS_EINVAL, "n_steps < 0");
+    const ts::Lattice3 L{plan->L.nx, plan->L.ny, plan->nz, plan->L.dtype,
+                         {plan->L.periodic_x, plan->L.periodic_y, plan->periodic_z}};
+    const size_t vol_bytes = (size_t)L.nx * (size_t)L.ny * (size_t)L.nz * plan->elem;
+    if (!aligned16(psi_re) || !aligned16(psi_im) || (pot && !aligned16(pot)))
+        return fail(TS_EINVAL, "device pointers must be 16-byte aligned");
+    if (overlap(psi_re, psi_im, vol_bytes)) return fail(TS_EINVAL, "psi_re and psi_im overlap");
+    if (pot && (overlap(pot, psi_re, vol_bytes) || overlap(pot, psi_im, vol_bytes) ||
+                overlap((const char*)pot + vol_bytes, psi_re, vol_bytes) ||
+                overlap((const char*)pot + vol_bytes, psi_im, vol_bytes)))
+        return fail(TS_EINVAL, "pot_phase overlaps psi");
+    if (!coef_ok(a_half, b_half) || !coef_ok(a_full, b_full))
+        return fail(TS_EINVAL, "coefficients must be finite with |a^2 + b^2 - 1| <= 1e-6");
+    const ts::StepCoef c{a_half, b_half, a_full, b_full};
+    const bool can_axis = ts::axis3_supported(L, c);
+    if ((plan->opt_path == 2 || plan->opt_variant == 4) && !can_axis)
+        return fail(TS_EUNSUPPORTED, "the fused 3-D path needs even extents that fit a thread block "
+                                     "(<= 16384 sites fp32, 8192 fp64, per axis) and cos of every "
+                                     "sweep angle > 0.25");
+    if (plan->opt_variant != 0 && plan->opt_variant != 4)
+        return fail(TS_EUNSUPPORTED, "3-D plans run on the axis path (variant 4) or the per-sweep kernels");
+    int rc = check_device(plan);
+    if (rc != TS_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    ts::LaunchTimer* tm = plan->opt_timing ? plan->timer : nullptr;
+    if (plan->timer) plan->timer->reset();
+    plan->info_fused = plan->info_fuse = plan->info_passes = plan->info_launches = 0;
+    plan->info_seg = plan->info_variant = plan->info_chain_x = plan->info_chain_y = 0;
+    if (n_steps == 0) return TS_OK;
+    if (can_axis && plan->opt_path != 1) {
+        ts::AxisInfo ai;
+        rc = ts::axis3_evolve(L, psi_re, psi_im, c, pot, n_steps, st, &ai, tm);
+        plan->info_launches = ai.launches;
+        if (rc != TS_OK) return rc;
+        plan->info_fused = 1; plan->info_passes = ai.passes; plan->info_variant = 4;
+        plan->info_chain_x = ai.chain_x; plan->info_chain_y = ai.chain_y;
+        plan->info_fuse = pot ? 1 : n_steps;
+        return TS_OK;
+    }
+    ts::timer_begin(tm, ts::kKindGeneric, st);
+    rc = ts::generic3_evolve(L, psi_re, psi_im, c, pot, n_steps, st, &plan->info_launches);
+    ts::timer_end(tm, st);
+    return rc;
+}
+
 int ts_evolve_sep(ts_plan* plan, void* psi_re, void* psi_im, double a_half, double b_half,
                   double a_full, double b_full, const void* phase_x, const void* phase_y,
                   int64_t n_steps, void* cuda_stream) {
@@ -419,6 +538,7 @@ int ts_slab_pass(ts_plan* plan, const void* src_re, const void* src_im, void* ds
                  int n_sub, const void* phase_x, const void* phase_y, int64_t y0,
                  int64_t ny_global, int periodic_y_global, void* cuda_stream) {
     if (!plan) return fail(TS_EINVAL, "NULL plan");
+    if (plan->nz != 1) return fail(TS_EINVAL, "three-dimensional plan: use ts_evolve_3d");
     if (!src_re || !src_im || !dst_re || !dst_im) return fail(TS_EINVAL, "NULL psi plane");
     if (!coef) return fail(TS_EINVAL, "NULL coefficient table");
     if ((up_re == nullptr) != (up_im == nullptr) || (dn_re == nullptr) != (dn_im == nullptr))
@@ -514,6 +634,43 @@ int ts_evolve_u4(ts_plan* plan, void* psi_re, void* psi_im, double theta, const 
     return evolve_pattern(plan, psi_re, psi_im, pat, 5, n_steps, cuda_stream);
 }
 
+int ts_plan_reserve(ts_plan* plan, int with_host_staging) {
+    if (!plan) return fail(TS_EINVAL, "NULL plan");
+    int rc = check_device(plan);
+    if (rc != TS_OK) return rc;
+    const size_t plane_bytes = (size_t)plan->L.nx * (size_t)plan->L.ny * plan->elem;
+    if (plan->nz == 1) {      // the 3-D paths work in place
+        rc = ensure_alloc(&plan->scratch_re, plane_bytes);
+        if (rc == TS_OK) rc = ensure_alloc(&plan->scratch_im, plane_bytes);
+    }
+    if (rc == TS_OK)
+        rc = ensure_alloc(reinterpret_cast<void**>(&plan->norm_work),
+                          ts::norm_workspace_doubles() * sizeof(double));
+    if (rc == TS_OK && with_host_staging) {
+        rc = ensure_alloc(&plan->host_re, plane_bytes);
+        if (rc == TS_OK) rc = ensure_alloc(&plan->host_im, plane_bytes);
+        if (rc == TS_OK && with_host_staging == 2) rc = ensure_alloc(&plan->host_pot, 2 * plane_bytes);
+    }
+    return rc;
+}
+
+int ts_plan_get_launch_times(ts_plan* plan, int max_n, int* kinds_out, float* ms_out, int* n_out) {
+    if (!plan || !n_out || max_n < 0 || (max_n > 0 && (!kinds_out || !ms_out)))
+        return fail(TS_EINVAL, "NULL argument");
+    *n_out = 0;
+    if (!plan->timer) return TS_OK;
+    const ts::LaunchTimer& t = *plan->timer;
+    *n_out = (int)t.used;
+    for (size_t i = 0; i < t.used && (int)i < max_n; ++i) {
+        TS_CUDA_TRY(cudaEventSynchronize(t.recs[i].b));
+        float ms = 0.f;
+        TS_CUDA_TRY(cudaEventElapsedTime(&ms, t.recs[i].a, t.recs[i].b));
+        kinds_out[i] = t.recs[i].kind;
+        ms_out[i] = ms;
+    }
+    return TS_OK;
+}
+
 int ts_norm(ts_plan* plan, const void* psi_re, const void* psi_im, double* out, void* cuda_stream) {
     if (!plan) return fail(TS_EINVAL, "NULL plan");
     if (!psi_re || !psi_im || !out) return fail(TS_EINVAL, "NULL argument");
@@ -523,7 +680,9 @@ int ts_norm(ts_plan* plan, const void* psi_re, const void* psi_im, double* out, 
     rc = ensure_alloc(reinterpret_cast<void**>(&plan->norm_work),
                       ts::norm_workspace_doubles() * sizeof(double));
     if (rc != TS_OK) return rc;
-    rc = ts::norm2_device(plan->L, psi_re, psi_im, plan->norm_work, st);
+    ts::LatticeDesc flat = plan->L;     // a 3-D state is nz * ny rows of nx sites
+    flat.ny *= plan->nz;
+    rc = ts::norm2_device(flat, psi_re, psi_im, plan->norm_work, st);
     if (rc != TS_OK) return rc;
     TS_CUDA_TRY(cudaMemcpyAsync(out, plan->norm_work, sizeof(double), cudaMemcpyDeviceToHost, st));
     TS_CUDA_TRY(cudaStreamSynchronize(st));

@@ -35,6 +35,7 @@
 // (sm_100 fma.rn.f32x2; ptxas folds the swapped source pair into an operand modifier).
 #include <math.h>
 #include <stdlib.h>
+#include <string.h>
 
 #include <atomic>
 #include <type_traits>
@@ -101,15 +102,49 @@ __device__ __forceinline__ void mulc(Cx<float>& p, float s) {
 // ---------------------------------------------------------------------------------------------
 // resident lines
 // ---------------------------------------------------------------------------------------------
+// In-place form of the pair rotation.  The from-old form above needs both old values for both
+// results, so a sweep over a lane's NS sites writes a second register set (ptxas ping-pongs two
+// full sets: 4 * NS registers in fp32, and the resident kernels spill).  Here the two sites of a
+// pair are updated one after the other, each in place:
+//
+//     first  += i k1 * second            second += i k2 * first(new)
+//
+// With the sites stored as actual = scale * stored, scale xi on the first and eta on the second
+// site, this is the rotation cos * [[1, i t],[i t, 1]] exactly when k1 = t eta / xi,
+// k2 = t cos^2 xi / eta, and the scales become cos * xi and eta / cos.  Even sweeps update the
+// even-index site first, odd sweeps the odd-index site, so over a sub-step (odd sweep + even sweep
+// of the same angle) the two scales return to where they were: nothing is deferred, nothing grows,
+// and the constants of uniform steps are the same in every sub-step.  All sites of one index
+// parity share one scale; the host follows the two scales in double (fill_chain) and the kernel
+// multiplies by what is left at the store.  Still two FMAs per site and sweep.
+constexpr int kMaxTab = 16;       // sub-steps per table cycle of a non-uniform pattern
+constexpr int kMaxProg = 4;       // sweeps of a sweep program
+
+template <typename T>
+struct SubCoef {   // one sub-step of a line chain: its odd sweep and the even sweep that follows it
+    T o1, o2;      // odd sweep: odd-index site += i o1 * partner, then even-index site += i o2 * partner'
+    // the even-index site of a cross-lane pair is computed from OLD values, second' = cos^2 second
+    // + i o2 first_old, and the unpaired sites of a closed line only follow their scale (site 0
+    // * cos, site n-1 / cos).  All three factors are 1 + (something tiny) and are applied as
+    // s += d * s: a factor rounded to T next to 1 is off by up to 3e-8, the same in every sweep,
+    // and the norm drifts (measured: -3e-5 over 100 steps on 64 x 64); d rounded to T is exact
+    // to 1e-7 * |d|.
+    T od2;         // -sin^2 = cos^2 - 1
+    T odc, ods;    // cos - 1, 1 / cos - 1
+    T e1, e2;      // the even sweep that follows: even-index site += i e1 * partner, then odd += i e2 * partner'
+};
+
 template <typename T>
 struct LineParams {
     const T* src_re;
     const T* src_im;
     T* dst_re;
     T* dst_im;
-    int64_t line_stride;    // elements between consecutive lines
+    int64_t line_stride;    // elements between consecutive lines of one group
     int64_t site_stride;    // elements between consecutive sites of a line (1: rows)
+    int64_t group_stride;   // elements between groups of lines_inner lines (3-D: planes)
     int n_lines, n_sites;
+    int lines_inner;        // lines per group (2-D: all of them)
     int n_lanes;            // one warp per line: lanes that hold sites (lines shorter than 32 * NS)
     int n_warps;            // warps per line (W); W > 1: every lane of every warp holds NS sites
     int lines_per_block;
@@ -117,14 +152,20 @@ struct LineParams {
     // windows (xwin_kernel only)
     int n_win, wi, halo, lines_per_warp;
     int64_t n_sub;          // sub-steps of this launch
-    int period, phase0;     // pattern of distinct sub-steps; index of this launch's first sub-step
-    int resc_every;         // deferred cosines are multiplied in every resc_every sub-steps ...
-    T resc;                 // ... by this factor (keeps the scaled amplitudes in range)
-    T final_scale;          // the rest of the deferred cosines, applied at the store
-    T te_first, te_last;    // tangents: opening and closing even half sweep
-    T te_mid[kMaxPeriod];   // even sweep merged from entry k's closing and entry k+1's opening half
-    T to[kMaxPeriod];       // odd sweep of pattern entry k
-    T sec_o[kMaxPeriod];    // 1 / cos of it (unpaired sites at closed ends)
+    int n_tab;              // sub-steps per table cycle; 1: uniform steps (constants in uniform registers)
+    int has_fix;            // after every cycle: s += fix * s per index parity (scales back to the cycle start)
+    T fix_e, fix_o;
+    T open1, open2;         // opening even half sweep
+    T close1, close2;       // closing even half sweep (replaces the even sweep of the last sub-step)
+    T fin_e, fin_o;         // what is left of the scales of even- / odd-index sites, applied at the store
+    SubCoef<T> tab[kMaxTab];
+    // sweep program (n_prog > 0, instead of a chain): up to kMaxProg sweeps with their own parity,
+    // then optionally the potential phase of the lane's sites (3-D steps with a potential)
+    int n_prog;
+    int prog_parity[kMaxProg];
+    SubCoef<T> prog[kMaxProg];      // odd sweep: o1, o2, od2, odc, ods; even sweep: e1, e2
+    const T* ph_re;
+    const T* ph_im;
 };
 
 template <typename T, int NS>
@@ -132,39 +173,68 @@ struct Line {
     Cx<T> s[NS];
 };
 
-template <typename T, int NS>
-__device__ __forceinline__ void line_even(Line<T, NS>& L, T t) {
-    const Coef<T> c = coef(t);
-#pragma unroll
-    for (int k = 0; k < NS; k += 2) rotc(L.s[k], L.s[k + 1], c);
+// first += i k1 second, then second += i k2 first (in place)
+template <typename T>
+__device__ __forceinline__ void rot_seq(Cx<T>& first, Cx<T>& second, T k1, T k2) {
+    rot1(first, second, coef(k1));
+    rot1(second, first, coef(k2));
+}
+// p += d * p
+template <typename T>
+__device__ __forceinline__ void fixc(Cx<T>& p, T d) {
+    p.re = fma(d, p.re, p.re); p.im = fma(d, p.im, p.im);
 }
 template <typename T, int NS>
-__device__ __forceinline__ void line_scale(Line<T, NS>& L, T s) {
+__device__ __forceinline__ void line_even_all(Line<T, NS>& L, T e1, T e2) {
 #pragma unroll
-    for (int k = 0; k < NS; ++k) mulc(L.s[k], s);
+    for (int k = 0; k < NS; k += 2) rot_seq(L.s[k], L.s[k + 1], e1, e2);
 }
-// the in-thread pairs (1,2), (3,4), ... of the odd sweep
+// the even pairs that do not contain the lane's first or last site
 template <typename T, int NS>
-__device__ __forceinline__ void line_odd_inner(Line<T, NS>& L, T t) {
-    const Coef<T> c = coef(t);
+__device__ __forceinline__ void line_even_mid(Line<T, NS>& L, T e1, T e2) {
 #pragma unroll
-    for (int k = 1; k + 1 < NS; k += 2) rotc(L.s[k], L.s[k + 1], c);
+    for (int k = 2; k + 2 < NS; k += 2) rot_seq(L.s[k], L.s[k + 1], e1, e2);
+}
+template <typename T, int NS>
+__device__ __forceinline__ void line_even_ends(Line<T, NS>& L, T e1, T e2) {
+    rot_seq(L.s[0], L.s[1], e1, e2);
+    if (NS > 2) rot_seq(L.s[NS - 2], L.s[NS - 1], e1, e2);
+}
+// the in-thread pairs (1,2), (3,4), ... of the odd sweep: the odd-index site goes first
+template <typename T, int NS>
+__device__ __forceinline__ void line_odd_inner(Line<T, NS>& L, T o1, T o2) {
+#pragma unroll
+    for (int k = 1; k + 1 < NS; k += 2) rot_seq(L.s[k], L.s[k + 1], o1, o2);
 }
 // the two sites whose partners (up: last site of the previous lane, dn: first site of the next)
-// live elsewhere.  EDGE: a pair may be cut (closed end, ghost lanes): its coupling is 0 and the
-// unpaired real site takes 1/cos of the omitted sweep instead (ts_rows.cuh).
+// live elsewhere, both taken BEFORE this sweep.  The last site (odd index) goes first in its pair
+// and uses the plain form; the first site (even index) goes second in its pair, whose other half
+// is updated by the neighbour, so it is computed from the old values:
+// second' = cos^2 second + i k2 first_old.  EDGE: a pair may be cut (closed end, ghost lanes): its
+// coupling is 0 and the unpaired site only follows its scale (site 0: * cos, last site: / cos).
 template <typename T, int NS, bool EDGE>
 __device__ __forceinline__ void line_odd_outer(Line<T, NS>& L, const Cx<T>& up, const Cx<T>& dn,
-                                               T t, T sec, bool cut_up, bool cut_dn) {
-    T t_up = t, t_dn = t;
+                                               const SubCoef<T>& c, bool cut_up, bool cut_dn) {
+    T k1 = c.o1, k2 = c.o2, d0 = c.od2;
     if (EDGE) {
-        t_up = cut_up ? T(0) : t;
-        t_dn = cut_dn ? T(0) : t;
-        mulc(L.s[0], cut_up ? sec : T(1));
-        mulc(L.s[NS - 1], cut_dn ? sec : T(1));
+        k1 = cut_dn ? T(0) : k1;
+        k2 = cut_up ? T(0) : k2;
+        d0 = cut_up ? c.odc : d0;
+        fixc(L.s[NS - 1], cut_dn ? c.ods : T(0));
     }
-    rot1(L.s[0], up, coef(t_up));
-    rot1(L.s[NS - 1], dn, coef(t_dn));
+    rot1(L.s[NS - 1], dn, coef(k1));
+    fixc(L.s[0], d0);
+    rot1(L.s[0], up, coef(k2));
+}
+template <typename T, int NS>
+__device__ __forceinline__ void line_scale2(Line<T, NS>& L, T fe, T fo) {
+#pragma unroll
+    for (int k = 0; k < NS; k += 2) { mulc(L.s[k], fe); mulc(L.s[k + 1], fo); }
+}
+template <typename T, int NS>
+__device__ __forceinline__ void line_fix(Line<T, NS>& L, T de, T dd) {
+#pragma unroll
+    for (int k = 0; k < NS; k += 2) { fixc(L.s[k], de); fixc(L.s[k + 1], dd); }
 }
 
 template <typename T>
@@ -192,37 +262,74 @@ __device__ __forceinline__ void st_piece(double* p, const double* v, int) {
     *reinterpret_cast<double2*>(p) = make_double2(v[0], v[1]);
 }
 
-// the chain E(h_0) O(f_0) E(h_0 + h_1) ... O(f_{n-1}) E(h_{n-1}) on the sites a lane holds;
-// pattern entry k = (phase0 + s) mod period.  `outer` supplies the cross-lane partners of one odd
-// sweep and applies them.  Uniform steps (period 1, ts_evolve) keep their three tangents in
-// uniform registers: a coefficient that is indexed by the running pattern position ends up in a
-// vector register instead, and a packed FMA with three vector-register sources issues at two
-// thirds of the rate.
-template <typename T, int NS, typename Outer>
-__device__ __forceinline__ void run_chain(const LineParams<T>& p, Line<T, NS>& L, Outer&& outer) {
-    line_even(L, p.te_first);
-    int since = 0;
-    if (p.period == 1) {
-        const T to = p.to[0], sec = p.sec_o[0], tm = p.te_mid[0];
+// The chain E(h_0) O(f_0) E(h_0 + h_1) ... O(f_{n-1}) E(h_{n-1}) on the sites a lane holds.  One
+// sub-step = an odd sweep and the even sweep after it, in the order that hides the exchange of the
+// two boundary sites: begin(L, up, dn) starts it (shuffles; several warps per line: publish +
+// arrive), the in-thread odd pairs and the even pairs that do not need the boundary sites follow,
+// end(up, dn) completes it (several warps: wait + pick up the neighbouring warps' sites), then the
+// two outer odd pairs and the two outer even pairs.  Uniform steps keep their constants in uniform
+// registers: a coefficient indexed by the running table position ends up in a vector register,
+// and a packed FMA with three vector-register sources issues at two thirds of the rate.
+template <typename T, int NS, bool EDGE, typename Begin, typename End>
+__device__ __forceinline__ void run_chain(const LineParams<T>& p, Line<T, NS>& L, bool cut_up,
+                                          bool cut_dn, Begin&& begin, End&& end) {
+    auto substep = [&](const SubCoef<T>& c, T e1, T e2) {
+        Cx<T> up, dn;
+        begin(L, up, dn);
+        line_odd_inner(L, c.o1, c.o2);
+        line_even_mid(L, e1, e2);
+        end(up, dn);
+        line_odd_outer<T, NS, EDGE>(L, up, dn, c, cut_up, cut_dn);
+        line_even_ends(L, e1, e2);
+    };
+    line_even_all(L, p.open1, p.open2);
+    if (p.n_tab == 1) {
+        const SubCoef<T> c = p.tab[0];
 #pragma unroll 1
-        for (int64_t s = 1; s < p.n_sub; ++s) {
-            outer(L, to, sec);
-            line_even(L, tm);
-            if (++since == p.resc_every) { since = 0; line_scale(L, p.resc); }
-        }
-        outer(L, to, sec);
+        for (int64_t s = 1; s < p.n_sub; ++s) substep(c, c.e1, c.e2);
+        substep(c, p.close1, p.close2);
     } else {
-        int k = p.phase0;
+        int j = 0;
 #pragma unroll 1
         for (int64_t s = 1; s < p.n_sub; ++s) {
-            outer(L, p.to[k], p.sec_o[k]);
-            line_even(L, p.te_mid[k]);
-            if (++k == p.period) k = 0;
-            if (++since == p.resc_every) { since = 0; line_scale(L, p.resc); }
+            const SubCoef<T> c = p.tab[j];
+            substep(c, c.e1, c.e2);
+            if (++j == p.n_tab) {
+                j = 0;
+                if (p.has_fix) line_fix(L, p.fix_e, p.fix_o);
+            }
         }
-        outer(L, p.to[k], p.sec_o[k]);
+        substep(p.tab[j], p.close1, p.close2);
     }
-    line_even(L, p.te_last);
+    line_scale2(L, p.fin_e, p.fin_o);
+}
+
+// A sweep program: a few sweeps with their own parities and angles (3-D steps with a potential:
+// O(h) E(f) O(h) between two applications of the phase).  The final scales are applied by the
+// caller after the phase.
+template <typename T, int NS, bool EDGE, typename Begin, typename End>
+__device__ __forceinline__ void run_prog(const LineParams<T>& p, Line<T, NS>& L, bool cut_up,
+                                         bool cut_dn, Begin&& begin, End&& end) {
+#pragma unroll 1
+    for (int i = 0; i < p.n_prog; ++i) {
+        const SubCoef<T> c = p.prog[i];
+        if (p.prog_parity[i] == 0) {
+            line_even_all(L, c.e1, c.e2);
+        } else {
+            Cx<T> up, dn;
+            begin(L, up, dn);
+            line_odd_inner(L, c.o1, c.o2);
+            end(up, dn);
+            line_odd_outer<T, NS, EDGE>(L, up, dn, c, cut_up, cut_dn);
+        }
+    }
+}
+// psi <- psi * (pr + i pi)
+template <typename T>
+__device__ __forceinline__ void phase_mul(Cx<T>& s, T pr, T pi) {
+    const T r = s.re, m = s.im;
+    s.re = fma(-m, pi, r * pr);
+    s.im = fma(m, pr, r * pi);
 }
 
 // COL = false: rows (site stride 1, 16-byte accesses); COL = true: columns (site stride = pitch,
@@ -265,7 +372,9 @@ line_kernel(const __grid_constant__ LineParams<T> p) {
 
     for (int line = blockIdx.x * p.lines_per_block + grp; line < p.n_lines;
          line += gridDim.x * p.lines_per_block) {
-        const int64_t base = (int64_t)line * p.line_stride;
+        const int grp_i = line / p.lines_inner;
+        const int64_t base = (int64_t)grp_i * p.group_stride +
+                             (int64_t)(line - grp_i * p.lines_inner) * p.line_stride;
         Line<T, NS> L;
         if (COL) {
 #pragma unroll
@@ -290,21 +399,21 @@ line_kernel(const __grid_constant__ LineParams<T> p) {
             }
         }
 
-        run_chain<T, NS>(p, L, [&](Line<T, NS>& M, T t, T sec) {
+        auto xbegin = [&](Line<T, NS>& M, Cx<T>& up, Cx<T>& dn) {
             if (MW) {
-                // publish the boundary sites (state after the even sweep), then the in-warp work,
-                // then pick up the neighbours' -- the wait overlaps the in-thread pairs
+                // publish the boundary sites (state after the even sweep); the wait for the
+                // neighbouring warps' comes after the in-thread work
                 if (lane == 0) xbuf[grp][par][wl][0] = M.s[0];
                 if (lane == 31) xbuf[grp][par][wl][1] = M.s[NS - 1];
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar);
             }
-            Cx<T> up, dn;
             up.re = __shfl_sync(0xffffffffu, M.s[NS - 1].re, up_src);
             up.im = __shfl_sync(0xffffffffu, M.s[NS - 1].im, up_src);
             dn.re = __shfl_sync(0xffffffffu, M.s[0].re, dn_src);
             dn.im = __shfl_sync(0xffffffffu, M.s[0].im, dn_src);
-            line_odd_inner(M, t);
+        };
+        auto xend = [&](Cx<T>& up, Cx<T>& dn) {
             if (MW) {
                 mbar_wait(bar, ph);
                 ph ^= 1;
@@ -313,10 +422,32 @@ line_kernel(const __grid_constant__ LineParams<T> p) {
                 if (lane == 31) dn = xbuf[grp][par][wd][0];
                 par ^= 1;
             }
-            line_odd_outer<T, NS, EDGE>(M, up, dn, t, sec, cut_up, cut_dn);
-        });
+        };
+        if (p.n_prog == 0) {
+            run_chain<T, NS, EDGE>(p, L, cut_up, cut_dn, xbegin, xend);
+        } else {
+            run_prog<T, NS, EDGE>(p, L, cut_up, cut_dn, xbegin, xend);
+            if (p.ph_re != nullptr && active) {
+                if (COL) {
+#pragma unroll
+                    for (int k = 0; k < NS; ++k) {
+                        const int64_t off = base + (int64_t)(xl + k) * p.site_stride;
+                        phase_mul(L.s[k], __ldg(p.ph_re + off), __ldg(p.ph_im + off));
+                    }
+                } else {
+#pragma unroll
+                    for (int k = 0; k < NS; k += PW) {
+                        T r[PW], i[PW];
+                        ld_piece(p.ph_re + base + xl + k, r, PW);
+                        ld_piece(p.ph_im + base + xl + k, i, PW);
+#pragma unroll
+                        for (int j = 0; j < PW; ++j) phase_mul(L.s[k + j], r[j], i[j]);
+                    }
+                }
+            }
+            line_scale2(L, p.fin_e, p.fin_o);
+        }
 
-        line_scale(L, p.final_scale);
         if (!active) continue;
         if (COL) {
 #pragma unroll
@@ -388,7 +519,6 @@ xwin_kernel(const __grid_constant__ LineParams<T> p) {
     };
     auto store = [&](int line, Line<T, NS>& L) {
         const int64_t base = (int64_t)line * p.line_stride;
-        line_scale(L, p.final_scale);
 #pragma unroll
         for (int k = 0; k < NS; k += PW) {
             const int x = xl + k;
@@ -402,15 +532,15 @@ xwin_kernel(const __grid_constant__ LineParams<T> p) {
         }
     };
     auto chain = [&](Line<T, NS>& L) {
-        run_chain<T, NS>(p, L, [&](Line<T, NS>& M, T t, T sec) {
-            Cx<T> up, dn;
-            up.re = __shfl_sync(0xffffffffu, M.s[NS - 1].re, up_src);
-            up.im = __shfl_sync(0xffffffffu, M.s[NS - 1].im, up_src);
-            dn.re = __shfl_sync(0xffffffffu, M.s[0].re, dn_src);
-            dn.im = __shfl_sync(0xffffffffu, M.s[0].im, dn_src);
-            line_odd_inner(M, t);
-            line_odd_outer<T, NS, EDGE>(M, up, dn, t, sec, cut_up, cut_dn);
-        });
+        run_chain<T, NS, EDGE>(
+            p, L, cut_up, cut_dn,
+            [&](Line<T, NS>& M, Cx<T>& up, Cx<T>& dn) {
+                up.re = __shfl_sync(0xffffffffu, M.s[NS - 1].re, up_src);
+                up.im = __shfl_sync(0xffffffffu, M.s[NS - 1].im, up_src);
+                dn.re = __shfl_sync(0xffffffffu, M.s[0].re, dn_src);
+                dn.im = __shfl_sync(0xffffffffu, M.s[0].im, dn_src);
+            },
+            [&](Cx<T>&, Cx<T>&) {});
     };
 
     Line<T, NS> A, B;
@@ -448,6 +578,25 @@ struct YcolParams {
     Coef<T> to[kMaxChain];       // odd sweep of sub-step j (the caller's full-angle coefficients)
     T sec_o[kMaxChain];
     T out_scale;
+    // uniform passes (UNI: S equal sub-steps, nothing padded): four coefficient pairs that stay in
+    // uniform registers instead of 2S + 1 pairs in vector registers
+    Coef<T> u_open, u_mid, u_odd, u_close;
+    T u_sec;
+};
+
+// coefficient of stage J: per-stage table, or the uniform pass's four pairs
+template <typename T, int S, bool UNI>
+struct YCoef {
+    static __device__ __forceinline__ Coef<T> even(const YcolParams<T>& p, int J) {
+        if (UNI) return J == 0 ? p.u_open : (J == S ? p.u_close : p.u_mid);
+        return p.te[J];
+    }
+    static __device__ __forceinline__ Coef<T> odd(const YcolParams<T>& p, int J) {
+        return UNI ? p.u_odd : p.to[J];
+    }
+    static __device__ __forceinline__ T sec(const YcolParams<T>& p, int J) {
+        return UNI ? p.u_sec : p.sec_o[J];
+    }
 };
 
 // stages 0..S-1 of one iteration.  Stage J holds the row pair that still waits for its odd
@@ -456,32 +605,33 @@ struct YcolParams {
 // the waiting pair's lower row with x0, and the waiting pair moves on to stage J+1.  Stage J owns
 // two register sets (ts_stream.cu: ping-pong form): the incoming pair is written to set u while
 // the pair that waited in set u^1 leaves.
-template <typename T, int S, bool EDGE, int J>
+template <typename T, int S, bool EDGE, bool UNI, int J>
 struct YStages {
     static __device__ __forceinline__ void run(const YcolParams<T>& p, int y, Cx<T> (&W)[S][2][2],
                                                const int u, Cx<T>& x0, Cx<T>& x1) {
+        using C = YCoef<T, S, UNI>;
         Cx<T>& a0 = W[J][u][0];
         Cx<T>& a1 = W[J][u][1];
         Cx<T>& g = W[J][u ^ 1][0];
         Cx<T>& h = W[J][u ^ 1][1];
         a0 = x0; a1 = x1;
-        rotc(a0, a1, p.te[J]);
+        rotc(a0, a1, C::even(p, J));
         if (EDGE) {
             // closed lattice: the odd pair (yj-1, yj) does not exist at yj = 0 and yj = ny; the
             // ghost row is zero and stays zero, the real row takes 1/cos of the omitted sweep
             const int yj = y - 2 * J;
             const bool yedge = yj == 0 || yj == p.ny;
-            Coef<T> c = p.to[J];
+            Coef<T> c = C::odd(p, J);
             if (yedge) { c.n = T(0); c.p = T(0); }
             rotc(h, a0, c);
-            const T sy = yedge ? p.sec_o[J] : T(1);
+            const T sy = yedge ? C::sec(p, J) : T(1);
             mulc(h, sy); mulc(a0, sy);
         } else {
-            rotc(h, a0, p.to[J]);
+            rotc(h, a0, C::odd(p, J));
         }
-        if (J == S - 1) rotc(g, h, p.te[S]);
+        if (J == S - 1) rotc(g, h, C::even(p, S));
         x0 = g; x1 = h;
-        if constexpr (J + 1 < S) YStages<T, S, EDGE, J + 1>::run(p, y, W, u, x0, x1);
+        if constexpr (J + 1 < S) YStages<T, S, EDGE, UNI, J + 1>::run(p, y, W, u, x0, x1);
     }
 };
 
@@ -509,17 +659,19 @@ __device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
 // resident blocks per SM the register budget of the pipeline allows: S waiting row pairs, the
 // incoming and the prefetched pair at 2 (fp32) / 4 (fp64) registers per site, ~64 for addresses,
 // counters and temporaries (ptxas -v)
-constexpr int ycol_blocks_for(int S, int words) {
+constexpr int ycol_blocks_for(int S, int words, bool uni) {
+    // uniform fp32 passes (ptxas -v: no spills at these caps); the others by estimate
+    if (uni && words == 1) return S <= 12 ? 4 : S <= 20 ? 3 : 2;
     const int est = (S + 3) * 4 * words + 64;
     return est <= 128 ? 4 : est <= 168 ? 3 : 2;
 }
-template <typename T, int S>
+template <typename T, int S, bool UNI>
 constexpr int ycol_min_blocks() {
-    return ycol_blocks_for(S, (int)(sizeof(T) / 4));
+    return ycol_blocks_for(S, (int)(sizeof(T) / 4), UNI);
 }
 
-template <typename T, int S, bool PERY>
-__global__ void __launch_bounds__(kYWarps * 32, ycol_min_blocks<T, S>())
+template <typename T, int S, bool PERY, bool UNI>
+__global__ void __launch_bounds__(kYWarps * 32, ycol_min_blocks<T, S, UNI>())
 ycol_kernel(const __grid_constant__ YcolParams<T> p) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr uint32_t ROWB = kYCols * sizeof(T);
@@ -629,7 +781,7 @@ ycol_kernel(const __grid_constant__ YcolParams<T> p) {
                 bool ready = true;
                 if (it + 2 < n_iter) ready = mbar_test(l_bar, l_ph);
                 Cx<T> x0 = cur[0], x1 = cur[1];
-                YStages<T, S, EDGE, 0>::run(p, y, W, U, x0, x1);
+                YStages<T, S, EDGE, UNI, 0>::run(p, y, W, U, x0, x1);
                 if (it >= 2 * S && lane_ok && y - 2 * S < y_out1) {
                     mulc(x0, p.out_scale); mulc(x1, p.out_scale);
                     o_re[0] = x0.re; o_im[0] = x0.im;
@@ -698,50 +850,78 @@ int sm_count() {
     return n;
 }
 
-// tangents and deferred cosines of a chain of n_sub sub-steps starting at pattern position first
+// Constants of a chain of n_sub sub-steps starting at pattern position `first`, for the in-place
+// form of the rotations (see SubCoef).  The host follows the scales of the even-index and the
+// odd-index sites (actual = scale * stored) in double through every sweep:
+//   even sweep, angle (c, t = tan):  k1 = t be / al,  k2 = t c^2 al / be,  al *= c,  be /= c
+//   odd sweep:                       k1 = t al / be,  k2 = t c^2 be / al,  be *= c,  al /= c
+// (al: even-index sites, be: odd-index sites).  Uniform steps: the scales return after every
+// sub-step (to rounding, which goes into the final scale) and one table entry serves all of them.
+// Other patterns: a table cycle of n_tab sub-steps, after which the stored values are corrected
+// by s += fix * s so that the scales are back at the start of the cycle (fix is tiny: the FMA form
+// keeps its rounding error ~1e-7 * |fix|).
 template <typename T>
 void fill_chain(LineParams<T>& p, const StepCoef* pat, int period, int64_t first, int64_t n_sub,
                 bool col) {
     p.n_sub = n_sub;
-    p.period = period;
-    p.phase0 = (int)(first % period);
-    const StepCoef& c_first = pat[first % period];
-    const StepCoef& c_last = pat[(first + n_sub - 1) % period];
-    p.te_first = (T)(c_first.b_h / c_first.a_h);
-    p.te_last = (T)(c_last.b_h / c_last.a_h);
-    double log_period = 0.0;       // log of the deferred cosines of one pattern period (odd + merged even)
-    for (int k = 0; k < kMaxPeriod; ++k) {
-        if (k < period) {
-            const Angle m = add(half_of(pat[k]), half_of(pat[(k + 1) % period]));
-            const Angle o = odd_of(pat[k], col);
-            p.te_mid[k] = (T)(m.s / m.c);
-            p.to[k] = (T)(o.s / o.c);
-            p.sec_o[k] = (T)(1.0 / o.c);
-            log_period += log(m.c) + log(o.c);
-        } else {
-            p.te_mid[k] = T(0); p.to[k] = T(0); p.sec_o[k] = T(1);
-        }
+    double al = 1.0, be = 1.0;
+    auto even_sweep = [&](const Angle& a, T& k1, T& k2) {
+        const double t = a.s / a.c, rho = be / al;
+        k1 = (T)(t * rho);
+        k2 = (T)(t * a.c * a.c / rho);
+        al *= a.c; be /= a.c;
+    };
+    auto odd_sweep = [&](const Angle& a, SubCoef<T>& sc) {
+        const double t = a.s / a.c, rho = al / be;
+        sc.o1 = (T)(t * rho);
+        sc.o2 = (T)(t * a.c * a.c / rho);
+        // cos - 1 without cancellation: -sin^2 / (1 + cos)
+        const double cm1 = -(a.s * a.s) / (1.0 + a.c);
+        sc.od2 = (T)(-(a.s * a.s));
+        sc.odc = (T)cm1;
+        sc.ods = (T)(-cm1 / a.c);
+        be *= a.c; al /= a.c;
+    };
+    auto entry = [&](int64_t s) -> const StepCoef& { return pat[(first + s) % period]; };
+    auto merged = [&](int64_t s) { return add(half_of(entry(s)), half_of(entry(s + 1))); };
+
+    even_sweep(half_of(entry(0)), p.open1, p.open2);
+    const double al0 = al, be0 = be;
+    // uniform: one pattern entry whose merged even angle is the odd angle (the scales then return
+    // after each sub-step up to the rounding of the caller's coefficients)
+    bool uniform = period == 1;
+    if (uniform) {
+        const Angle m = merged(0), o = odd_of(entry(0), col);
+        uniform = fabs(m.c / o.c - 1.0) < 1e-12;
     }
-    // total: cos(opening half) * prod over sub-steps of cos(odd) * cos(following even sweep); the
-    // last even sweep is the closing half sweep, not a merged one.  Pattern entry k occurs
-    // cnt[k] times among the n_sub sub-steps (n_sub may be millions: no loop over them).
-    double log_total = log(c_first.a_h) + log(c_last.a_h);
-    const int k_last = (int)((first + n_sub - 1) % period);
-    for (int k = 0; k < period; ++k) {
-        const int64_t r = ((k - first) % period + period) % period;     // first s with entry k
-        const int64_t cnt = r < n_sub ? (n_sub - r + period - 1) / period : 0;
-        const Angle m = add(half_of(pat[k]), half_of(pat[(k + 1) % period]));
-        const Angle o = odd_of(pat[k], col);
-        log_total += (double)cnt * log(o.c) + (double)(cnt - (k == k_last ? 1 : 0)) * log(m.c);
+    p.n_tab = uniform ? 1 : period * (kMaxTab / period);
+    for (int j = 0; j < kMaxTab; ++j) p.tab[j] = SubCoef<T>{T(0), T(0), T(0), T(0), T(0), T(0), T(0)};
+    for (int j = 0; j < p.n_tab; ++j) {
+        odd_sweep(odd_of(entry(j), col), p.tab[j]);
+        even_sweep(merged(j), p.tab[j].e1, p.tab[j].e2);
     }
-    // every resc_every sub-steps (a multiple of the period: the factor is then the same each
-    // time) the kernel multiplies by resc; what is left goes into final_scale, together with the
-    // accumulated rounding error of resc
-    const int every = period * ((8 + period - 1) / period);
-    p.resc_every = every;
-    p.resc = (T)exp(log_period * (every / period));
-    const int64_t n_resc = (n_sub - 1) / every;      // the last sub-step is outside the loop
-    p.final_scale = (T)exp(log_total - (double)n_resc * log((double)p.resc));
+    // one cycle multiplies the scales by (ce, co); the fix takes that out of the stored values
+    const double ce = al / al0, co = be / be0;
+    p.has_fix = uniform ? 0 : 1;
+    p.fix_e = uniform ? T(0) : (T)(ce - 1.0);
+    p.fix_o = uniform ? T(0) : (T)(co - 1.0);
+    // what a cycle really leaves behind (the fix is rounded to T; uniform: no fix at all)
+    const double ge = ce / (1.0 + (double)p.fix_e), go = co / (1.0 + (double)p.fix_o);
+    const int64_t n_cycles = (n_sub - 1) / p.n_tab;       // complete cycles before the last sub-step
+    const int64_t rest = (n_sub - 1) - n_cycles * p.n_tab;
+    // the last, partial cycle with the table's own (nominal) scales: `rest` whole sub-steps, then
+    // the odd sweep of the last sub-step and the closing half sweep
+    al = al0; be = be0;
+    SubCoef<T> scratch;
+    T k1, k2;
+    for (int64_t j = 0; j < rest; ++j) {
+        odd_sweep(odd_of(entry(j), col), scratch);
+        even_sweep(merged(j), k1, k2);
+    }
+    odd_sweep(odd_of(entry(rest), col), scratch);
+    even_sweep(half_of(entry(n_sub - 1)), p.close1, p.close2);
+    p.fin_e = (T)(al * exp((double)n_cycles * log(ge)));
+    p.fin_o = (T)(be * exp((double)n_cycles * log(go)));
 }
 
 template <typename T, int NS, bool EDGE, bool COL, bool MW>
@@ -782,26 +962,39 @@ int launch_line_t(const LineParams<T>& p, int ns, bool edge, bool col, cudaStrea
     return TS_EUNSUPPORTED;
 }
 
-// One launch of the line kernel: ALL n_sub sub-steps of the pattern along the rows (col = false)
-// or the columns, in place.
+// Where the lines of one launch lie: line l = group g = l / lines_inner, member m = l % lines_inner
+// starts at g * group_stride + m * line_stride; consecutive sites are site_stride apart.
+struct LineGeom {
+    int64_t n_sites;
+    int periodic;
+    int64_t n_lines, line_stride, site_stride, lines_inner, group_stride;
+    bool col;              // site_stride != 1: scalar accesses, adjacent lines in one block
+};
+LineGeom rows_of(const LatticeDesc& L) {
+    return LineGeom{L.nx, L.periodic_x, L.ny, L.nx, 1, L.ny, 0, false};
+}
+LineGeom cols_of(const LatticeDesc& L) {
+    return LineGeom{L.ny, L.periodic_y, L.nx, 1, L.nx, L.nx, 0, true};
+}
+
+// launch the line kernel on lines held completely in registers; p carries a chain (fill_chain) or
+// a sweep program (fill_prog)
 template <typename T>
-int line_pass(const LatticeDesc& L, T* re, T* im, const StepCoef* pat, int period, int64_t n_sub,
-              bool col, cudaStream_t st) {
-    LineParams<T> p = {};
+int launch_lines(const LineGeom& g, int dtype, LineParams<T>& p, T* re, T* im, cudaStream_t st) {
     p.src_re = re; p.src_im = im; p.dst_re = re; p.dst_im = im;
-    const int64_t n = col ? L.ny : L.nx;
-    const bool periodic = col ? L.periodic_y : L.periodic_x;
-    p.n_lines = (int)(col ? L.nx : L.ny);
-    p.n_sites = (int)n;
-    p.line_stride = col ? 1 : L.nx;
-    p.site_stride = col ? L.nx : 1;
-    p.periodic = periodic;
-    const LineShape sh = line_shape(n, L.dtype);
+    p.n_lines = (int)g.n_lines;
+    p.n_sites = (int)g.n_sites;
+    p.line_stride = g.line_stride;
+    p.site_stride = g.site_stride;
+    p.lines_inner = (int)g.lines_inner;
+    p.group_stride = g.group_stride;
+    p.periodic = g.periodic;
+    const LineShape sh = line_shape(g.n_sites, dtype);
     if (!sh.ok()) { set_error("axis: line does not fit a thread block"); return TS_EUNSUPPORTED; }
     p.n_lanes = sh.lanes;
     p.n_warps = sh.warps;
     if (sh.warps == 1) {
-        // 4 lines per block; columns: 8, so that a block covers whole 32-byte sectors in fp32
+        // 4 lines per block (adjacent columns share their 32-byte sectors)
         p.lines_per_block = 4;
         const int64_t want = ((int64_t)p.n_lines + sm_count() * 4 - 1) / (sm_count() * 4);
         if (want < 4) p.lines_per_block = want < 1 ? 1 : (int)want;
@@ -809,9 +1002,55 @@ int line_pass(const LatticeDesc& L, T* re, T* im, const StepCoef* pat, int perio
         p.lines_per_block = 1;
         if (sh.warps <= 8) p.lines_per_block = 4 / sh.warps > 1 ? 4 / sh.warps : 1;
     }
+    const bool edge = !g.periodic || sh.lanes < 32;
+    return launch_line_t<T>(p, sh.ns, edge, g.col, st);
+}
+
+// One launch of the line kernel: ALL n_sub sub-steps of the pattern along the rows (col = false)
+// or the columns, in place.
+template <typename T>
+int line_pass(const LatticeDesc& L, T* re, T* im, const StepCoef* pat, int period, int64_t n_sub,
+              bool col, cudaStream_t st) {
+    LineParams<T> p = {};
     fill_chain(p, pat, period, 0, n_sub, col);
-    const bool edge = !periodic || sh.lanes < 32;
-    return launch_line_t<T>(p, sh.ns, edge, col, st);
+    return launch_lines<T>(col ? cols_of(L) : rows_of(L), L.dtype, p, re, im, st);
+}
+
+// Constants of a sweep program: sweeps (parity, angle) applied in order, scales followed as in
+// fill_chain; phase planes (or null) multiplied in after the last sweep.
+struct ProgStep {
+    int parity;
+    Angle a;
+};
+template <typename T>
+void fill_prog(LineParams<T>& p, const ProgStep* steps, int n, const T* ph_re, const T* ph_im) {
+    double al = 1.0, be = 1.0;
+    p.n_prog = n;
+    p.n_sub = 0; p.n_tab = 1;
+    for (int i = 0; i < n; ++i) {
+        const Angle& a = steps[i].a;
+        const double t = a.s / a.c;
+        SubCoef<T> sc = {};
+        p.prog_parity[i] = steps[i].parity;
+        if (steps[i].parity == 0) {
+            const double rho = be / al;
+            sc.e1 = (T)(t * rho);
+            sc.e2 = (T)(t * a.c * a.c / rho);
+            al *= a.c; be /= a.c;
+        } else {
+            const double rho = al / be;
+            const double cm1 = -(a.s * a.s) / (1.0 + a.c);
+            sc.o1 = (T)(t * rho);
+            sc.o2 = (T)(t * a.c * a.c / rho);
+            sc.od2 = (T)(-(a.s * a.s));
+            sc.odc = (T)cm1;
+            sc.ods = (T)(-cm1 / a.c);
+            be *= a.c; al /= a.c;
+        }
+        p.prog[i] = sc;
+    }
+    p.fin_e = (T)al; p.fin_o = (T)be;
+    p.ph_re = ph_re; p.ph_im = ph_im;
 }
 
 // One windowed pass along the rows: sub-steps [first, first + n_sub), n_sub <= kMaxChain, out of
@@ -825,6 +1064,8 @@ int xwin_pass(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re,
     p.n_sites = (int)L.nx;
     p.line_stride = L.nx;
     p.site_stride = 1;
+    p.lines_inner = p.n_lines;
+    p.group_stride = 0;
     p.periodic = L.periodic_x;
     constexpr int ns = sizeof(T) == 4 ? 32 : 16;
     // the halo: 2 sites per sub-step; lane-aligned on a closed row so that its ends fall between
@@ -847,11 +1088,11 @@ int xwin_pass(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re,
     return TS_OK;
 }
 
-template <typename T, int S, bool PERY>
+template <typename T, int S, bool PERY, bool UNI>
 int launch_ycol(const YcolParams<T>& p, cudaStream_t st) {
     constexpr uint32_t SLOTB = 4 * kYCols * sizeof(T);
     const size_t smem = (size_t)kYWarps * p.nst * (SLOTB + 8);
-    auto kern = ycol_kernel<T, S, PERY>;
+    auto kern = ycol_kernel<T, S, PERY, UNI>;
     static std::atomic<size_t> configured[64];
     int dev = 0;
     TS_CUDA_TRY(cudaGetDevice(&dev));
@@ -871,14 +1112,16 @@ int launch_ycol(const YcolParams<T>& p, cudaStream_t st) {
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     // as in ts_stream.cu: dependent launch only for grids of at most one wave
-    cfg.numAttrs = ((int64_t)grid.x * grid.y <= (int64_t)sm_count() * ycol_min_blocks<T, S>()) ? 1 : 0;
+    cfg.numAttrs = ((int64_t)grid.x * grid.y <= (int64_t)sm_count() * ycol_min_blocks<T, S, UNI>()) ? 1 : 0;
     TS_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, p));
     return TS_OK;
 }
 
 template <typename T, int S>
-int launch_ycol_s(const YcolParams<T>& p, cudaStream_t st) {
-    return p.periodic_y ? launch_ycol<T, S, true>(p, st) : launch_ycol<T, S, false>(p, st);
+int launch_ycol_s(const YcolParams<T>& p, bool uni, cudaStream_t st) {
+    if (uni)
+        return p.periodic_y ? launch_ycol<T, S, true, true>(p, st) : launch_ycol<T, S, false, true>(p, st);
+    return p.periodic_y ? launch_ycol<T, S, true, false>(p, st) : launch_ycol<T, S, false, false>(p, st);
 }
 
 // pipeline depths that are instantiated: the smallest one that holds n sub-steps
@@ -891,7 +1134,7 @@ int ycol_depth(int n, int dtype) {
         if (n <= d[i]) return d[i];
     return d[nd - 1];
 }
-int ycol_blocks_per_sm(int S, int dtype) { return ycol_blocks_for(S, dtype == TS_F32 ? 1 : 2); }
+int ycol_blocks_per_sm(int S, int dtype, bool uni) { return ycol_blocks_for(S, dtype == TS_F32 ? 1 : 2, uni); }
 
 // One pipelined pass along the columns: sub-steps subs[0 .. n) chained, padded with identity
 // sub-steps (zero angle) up to the instantiated depth S.
@@ -924,13 +1167,20 @@ int ycol_pass(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re,
     p.te[S] = Coef<T>{-tl, tl};
     log_scale += log(prev.c);
     p.out_scale = (T)exp(log_scale);
+    // S equal sub-steps and nothing padded: the coefficients are four pairs
+    bool uni = n == S && S > 1;
+    for (int j = 1; j < n && uni; ++j) uni = memcmp(&subs[j], &subs[0], sizeof(StepCoef)) == 0;
+    if (uni) {
+        p.u_open = p.te[0]; p.u_mid = p.te[1]; p.u_odd = p.to[0]; p.u_close = p.te[S];
+        p.u_sec = p.sec_o[0];
+    }
     switch (S) {
-        case 4: return launch_ycol_s<T, 4>(p, st);
-        case 8: return launch_ycol_s<T, 8>(p, st);
-        case 12: return launch_ycol_s<T, 12>(p, st);
-        case 16: if constexpr (sizeof(T) == 4) return launch_ycol_s<T, 16>(p, st); break;
-        case 20: if constexpr (sizeof(T) == 4) return launch_ycol_s<T, 20>(p, st); break;
-        case 24: if constexpr (sizeof(T) == 4) return launch_ycol_s<T, 24>(p, st); break;
+        case 4: return launch_ycol_s<T, 4>(p, uni, st);
+        case 8: return launch_ycol_s<T, 8>(p, uni, st);
+        case 12: return launch_ycol_s<T, 12>(p, uni, st);
+        case 16: if constexpr (sizeof(T) == 4) return launch_ycol_s<T, 16>(p, uni, st); break;
+        case 20: if constexpr (sizeof(T) == 4) return launch_ycol_s<T, 20>(p, uni, st); break;
+        case 24: if constexpr (sizeof(T) == 4) return launch_ycol_s<T, 24>(p, uni, st); break;
     }
     set_error("axis: pipeline depth not instantiated");
     return TS_EINVAL;
@@ -940,10 +1190,10 @@ int ycol_pass(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re,
 // segments win until the grid no longer fills the machine evenly.  Among the segment counts that
 // give at most `cap` rows, take the one with the smallest makespan (waves of resident blocks x
 // rows per block).
-int ycol_default_seg(const LatticeDesc& L, int S) {
+int ycol_default_seg(const LatticeDesc& L, int S, bool uni) {
     const int64_t strips = (L.nx + kYCols - 1) / kYCols;
     const int64_t blocks_x = (strips + kYWarps - 1) / kYWarps;
-    const int64_t slots = (int64_t)sm_count() * ycol_blocks_per_sm(S, L.dtype);
+    const int64_t slots = (int64_t)sm_count() * ycol_blocks_per_sm(S, L.dtype, uni);
     const int64_t cap = 4096;
     int64_t best_seg = L.ny, best_cost = -1;
     for (int64_t segs = 1; segs <= L.ny / 2; ++segs) {
@@ -991,7 +1241,7 @@ int axis_default_chain(const LatticeDesc& L) {
 template <typename T>
 static int axis_evolve_t(const LatticeDesc& L, T* psi_re, T* psi_im, T* scr_re, T* scr_im,
                          const StepCoef* pat, int period, int64_t n_sub, int chain, int seg_rows,
-                         int nst, cudaStream_t st, AxisInfo* info) {
+                         int nst, cudaStream_t st, AxisInfo* info, LaunchTimer* tm) {
     T* cur_re = psi_re; T* cur_im = psi_im;
     T* nxt_re = scr_re; T* nxt_im = scr_im;
     auto flip = [&]() {
@@ -1005,7 +1255,9 @@ static int axis_evolve_t(const LatticeDesc& L, T* psi_re, T* psi_im, T* scr_re, 
     int rc;
     // ---- rows
     if (x_res) {
+        timer_begin(tm, kKindLineRows, st);
         rc = line_pass<T>(L, cur_re, cur_im, pat, period, n_sub, false, st);
+        timer_end(tm, st);
         if (rc != TS_OK) return rc;
         ++info->passes; ++info->launches;
         info->chain_x = n_sub;
@@ -1013,7 +1265,9 @@ static int axis_evolve_t(const LatticeDesc& L, T* psi_re, T* psi_im, T* scr_re, 
         const int sx = chain < kMaxChain ? chain : kMaxChain;
         for (int64_t i = 0; i < n_sub; i += sx) {
             const int64_t s = n_sub - i < sx ? n_sub - i : sx;
+            timer_begin(tm, kKindXwin, st);
             rc = xwin_pass<T>(L, cur_re, cur_im, nxt_re, nxt_im, pat, period, i, s, st);
+            timer_end(tm, st);
             if (rc != TS_OK) return rc;
             flip();
             ++info->passes; ++info->launches;
@@ -1022,7 +1276,9 @@ static int axis_evolve_t(const LatticeDesc& L, T* psi_re, T* psi_im, T* scr_re, 
     }
     // ---- columns
     if (y_res) {
+        timer_begin(tm, kKindLineCols, st);
         rc = line_pass<T>(L, cur_re, cur_im, pat, period, n_sub, true, st);
+        timer_end(tm, st);
         if (rc != TS_OK) return rc;
         ++info->passes; ++info->launches;
         info->chain_y = n_sub;
@@ -1030,32 +1286,50 @@ static int axis_evolve_t(const LatticeDesc& L, T* psi_re, T* psi_im, T* scr_re, 
         const int smax = ycol_depth(kMaxChain, L.dtype);
         int want = (int)(n_sub < chain ? n_sub : chain);
         if (want > smax) want = smax;
-        // equal passes: 200 sub-steps at depth 24 are 9 passes of 22 or 23, not 8 of 24 and one of 8
-        const int64_t n_pass = (n_sub + want - 1) / want;
-        const int per_pass = (int)((n_sub + n_pass - 1) / n_pass);
-        const int S = ycol_depth(per_pass, L.dtype);
-        const int seg = seg_rows > 0 ? seg_rows : ycol_default_seg(L, S);
         // ring slots per warp: at least 3 (iteration i+2 is waited for while slot i-1 is the one
         // being refilled), at most what 200 KB of shared memory per block hold
         int slots = nst >= 3 ? nst : (nst > 0 ? 3 : 8);
         const int slot_max = (int)((200 << 10) / (kYWarps * (4 * kYCols * sizeof(T) + 8)));
         if (slots > slot_max) slots = slot_max;
         StepCoef subs[kMaxChain];
-        for (int64_t i = 0; i < n_sub; i += per_pass) {
-            const int s = (int)(n_sub - i < per_pass ? n_sub - i : per_pass);
+        int64_t i = 0;
+        while (i < n_sub) {
+            int s, S;
+            if (period == 1) {
+                // uniform steps: passes of exactly an instantiated depth run on the kernel whose
+                // coefficients stay in uniform registers (200 = 8 x 24 + 8); what is left below
+                // the smallest depth is one padded pass
+                const int64_t left = n_sub - i;
+                const int cap = (int)(left < want ? left : want);
+                S = ycol_depth(cap, L.dtype);
+                if (S > cap && cap >= 4) S = cap / 4 * 4;       // depths are the multiples of 4
+                s = S < cap ? S : cap;
+            } else {
+                // equal passes: 200 sub-steps at depth 24 are 9 passes of 22 or 23
+                const int64_t n_pass = (n_sub + want - 1) / want;
+                const int per_pass = (int)((n_sub + n_pass - 1) / n_pass);
+                S = ycol_depth(per_pass, L.dtype);
+                s = (int)(n_sub - i < per_pass ? n_sub - i : per_pass);
+            }
             for (int j = 0; j < s; ++j) subs[j] = pat[(i + j) % period];
+            const bool uni = period == 1 && s == S && S > 1;
+            const int seg = seg_rows > 0 ? seg_rows : ycol_default_seg(L, S, uni);
+            timer_begin(tm, kKindYcol, st);
             rc = ycol_pass<T>(L, cur_re, cur_im, nxt_re, nxt_im, subs, s, S, seg, slots, st);
+            timer_end(tm, st);
             if (rc != TS_OK) return rc;
             flip();
             ++info->passes; ++info->launches;
+            if (i == 0) { info->chain_y = s; info->seg_rows = seg; }
+            i += s;
         }
-        info->chain_y = per_pass;
-        info->seg_rows = seg;
     }
     if (cur_re != psi_re) {
         const size_t plane_bytes = (size_t)L.nx * (size_t)L.ny * sizeof(T);
+        timer_begin(tm, kKindCopy, st);
         TS_CUDA_TRY(cudaMemcpyAsync(psi_re, cur_re, plane_bytes, cudaMemcpyDeviceToDevice, st));
         TS_CUDA_TRY(cudaMemcpyAsync(psi_im, cur_im, plane_bytes, cudaMemcpyDeviceToDevice, st));
+        timer_end(tm, st);
         info->launches += 2;
     }
     return TS_OK;
@@ -1067,15 +1341,93 @@ bool axis_needs_scratch(const LatticeDesc& L) {
 
 int axis_evolve(const LatticeDesc& L, void* psi_re, void* psi_im, void* scr_re, void* scr_im,
                 const StepCoef* pat, int period, int64_t n_sub, int chain, int seg_rows, int nst,
-                cudaStream_t st, AxisInfo* info) {
+                cudaStream_t st, AxisInfo* info, LaunchTimer* tm) {
     if (chain <= 0) chain = axis_default_chain(L);
     if (L.dtype == TS_F32)
         return axis_evolve_t<float>(L, (float*)psi_re, (float*)psi_im, (float*)scr_re,
                                     (float*)scr_im, pat, period, n_sub, chain, seg_rows, nst, st,
-                                    info);
+                                    info, tm);
     return axis_evolve_t<double>(L, (double*)psi_re, (double*)psi_im, (double*)scr_re,
                                  (double*)scr_im, pat, period, n_sub, chain, seg_rows, nst, st,
-                                 info);
+                                 info, tm);
+}
+
+
+// ---- three-dimensional lattices (ts_internal.h) -------------------------------------------------------
+// psi[nz][ny][nx]: the step Xe Xo Ye Yo Ze [Zo | Zo P Zo] Ze Yo Ye Xo Xe.  Sweeps
+// along different axes commute, so without a potential n steps are three chains (one launch per
+// axis with every line resident in registers), and with one the sweeps between two applications of
+// the phase regroup per axis into O(h) E(2h) O(h):
+//   [X: E O] [Y: E O] [Z: E O, P]  { [X: O E O] [Y: O E O] [Z: O E O, P] }^(n-1)  [Z: O E] [Y: O E] [X: O E]
+// -- three launches per step, 16 B per site each (+ 8 B phase on the z launch, fp32) instead of
+// thirteen sweeps.
+namespace {
+LineGeom geom3(const Lattice3& L, int axis) {
+    const int64_t plane = L.nx * L.ny;
+    if (axis == 0) return LineGeom{L.nx, L.per[0], L.ny * L.nz, L.nx, 1, L.ny * L.nz, 0, false};
+    if (axis == 1) return LineGeom{L.ny, L.per[1], L.nx * L.nz, 1, L.nx, L.nx, plane, true};
+    return LineGeom{L.nz, L.per[2], plane, 1, plane, plane, 0, true};
+}
+const int kKindOfAxis[3] = {kKindLineRows, kKindLineCols, kKindLineZ};
+
+template <typename T>
+int axis3_evolve_t(const Lattice3& L, T* re, T* im, const StepCoef& c, const T* pot,
+                   int64_t n_steps, cudaStream_t st, AxisInfo* info, LaunchTimer* tm) {
+    info->passes = info->launches = 0;
+    info->chain_x = info->chain_y = n_steps; info->seg_rows = 0;
+    int rc;
+    if (pot == nullptr) {
+        for (int axis = 0; axis < 3; ++axis) {
+            LineParams<T> p = {};
+            fill_chain(p, &c, 1, 0, n_steps, /*innermost axis: the caller's full angle*/ axis == 2);
+            timer_begin(tm, kKindOfAxis[axis], st);
+            rc = launch_lines<T>(geom3(L, axis), L.dtype, p, re, im, st);
+            timer_end(tm, st);
+            if (rc != TS_OK) return rc;
+            ++info->passes; ++info->launches;
+        }
+        return TS_OK;
+    }
+    const Angle h = half_of(c), f = add(h, h);
+    const int64_t sites = L.nx * L.ny * L.nz;
+    auto run = [&](int axis, const ProgStep* steps, int n, bool phase) -> int {
+        LineParams<T> p = {};
+        fill_prog<T>(p, steps, n, phase ? pot : nullptr, phase ? pot + sites : nullptr);
+        timer_begin(tm, kKindOfAxis[axis], st);
+        const int r = launch_lines<T>(geom3(L, axis), L.dtype, p, re, im, st);
+        timer_end(tm, st);
+        ++info->passes; ++info->launches;
+        return r;
+    };
+    const ProgStep open[2] = {{0, h}, {1, h}};
+    const ProgStep mid[3] = {{1, h}, {0, f}, {1, h}};
+    const ProgStep close[2] = {{1, h}, {0, h}};
+    for (int axis = 0; axis < 3; ++axis)
+        if ((rc = run(axis, open, 2, axis == 2)) != TS_OK) return rc;
+    for (int64_t s = 1; s < n_steps; ++s)
+        for (int axis = 0; axis < 3; ++axis)
+            if ((rc = run(axis, mid, 3, axis == 2)) != TS_OK) return rc;
+    for (int axis = 2; axis >= 0; --axis)
+        if ((rc = run(axis, close, 2, false)) != TS_OK) return rc;
+    return TS_OK;
+}
+}  // namespace
+
+bool axis3_supported(const Lattice3& L, const StepCoef& c) {
+    const Angle h = half_of(c), f = add(h, h);
+    if (!(c.a_h > 0.25 && c.a_f > 0.25 && f.c > 0.25)) return false;
+    const int64_t n[3] = {L.nx, L.ny, L.nz};
+    for (int a = 0; a < 3; ++a)
+        if (n[a] < 2 || n[a] >= (int64_t(1) << 30) || !line_shape(n[a], L.dtype).ok()) return false;
+    return L.nx * L.ny < (int64_t(1) << 31) && L.ny * L.nz < (int64_t(1) << 31) &&
+           L.nx * L.nz < (int64_t(1) << 31);
+}
+
+int axis3_evolve(const Lattice3& L, void* re, void* im, const StepCoef& c, const void* pot,
+                 int64_t n_steps, cudaStream_t st, AxisInfo* info, LaunchTimer* tm) {
+    if (L.dtype == TS_F32)
+        return axis3_evolve_t<float>(L, (float*)re, (float*)im, c, (const float*)pot, n_steps, st, info, tm);
+    return axis3_evolve_t<double>(L, (double*)re, (double*)im, c, (const double*)pot, n_steps, st, info, tm);
 }
 
 }  // namespace ts

@@ -241,6 +241,89 @@ int expand_separable(const LatticeDesc& L, const void* px, const void* py, void*
     return TS_OK;
 }
 
+
+// ---- three-dimensional lattices: one launch per sweep ----------------------------------------------
+// psi[nz][ny][nx]; a sweep along an axis of extent n whose sites are `m` elements apart (x: 1,
+// y: nx, z: nx*ny) on `outer` repetitions (x: ny*nz, y: nz, z: 1): element (o, i, r) at
+// (o*n + i)*m + r.  Pair k of a line couples i = parity + 2k and i + 1 (or the wrap pair).
+namespace {
+template <typename T>
+__global__ void __launch_bounds__(256)
+sweep3_kernel(T* __restrict__ re, T* __restrict__ im, int64_t m, int64_t n, int64_t outer,
+              int parity, int64_t pairs, int wrap, RotCoef<T> c) {
+    const int64_t total = pairs * m * outer;
+    for (int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; t < total;
+         t += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t r = t % m;
+        const int64_t q1 = t / m;
+        const int64_t k = q1 % pairs;
+        const int64_t o = q1 / pairs;
+        const int64_t i = parity + 2 * k;
+        const int64_t p = (o * n + i) * m + r;
+        const int64_t q = (wrap && i == n - 1) ? (o * n) * m + r : p + m;
+        rotate(re, im, p, q, c);
+    }
+}
+
+template <typename T>
+int sweep3(const Lattice3& L, T* re, T* im, int axis, int parity, double a, double b,
+           cudaStream_t st, int64_t* launches) {
+    const int64_t n = axis == 0 ? L.nx : (axis == 1 ? L.ny : L.nz);
+    const int64_t m = axis == 0 ? 1 : (axis == 1 ? L.nx : L.nx * L.ny);
+    const int64_t outer = axis == 0 ? L.ny * L.nz : (axis == 1 ? L.nz : 1);
+    const int wrap = (L.per[axis] && parity == 1) ? 1 : 0;
+    int64_t pairs = parity == 0 ? n / 2 : (n - 1) / 2;
+    if (wrap) pairs += 1;
+    if (pairs <= 0) return TS_OK;
+    const RotCoef<T> c = make_rot<T>(a, b);
+    const int64_t total = pairs * m * outer;
+    sweep3_kernel<T><<<grid_for(total, 256), 256, 0, st>>>(re, im, m, n, outer, parity, pairs, wrap, c);
+    ++*launches;
+    TS_CUDA_TRY(cudaGetLastError());
+    return TS_OK;
+}
+
+// the literal stage list of the 3-D step (include/ts.h, ts_evolve_3d)
+template <typename T>
+int evolve3_t(const Lattice3& L, T* re, T* im, const StepCoef& c, const T* pot, int64_t n_steps,
+              cudaStream_t st, int64_t* launches) {
+    const int64_t sites = L.nx * L.ny * L.nz;
+    int rc;
+#define TS_SWEEP3(axis, parity, a, b)                                                        \
+    if ((rc = sweep3<T>(L, re, im, axis, parity, a, b, st, launches)) != TS_OK) return rc
+    for (int64_t s = 0; s < n_steps; ++s) {
+        TS_SWEEP3(0, 0, c.a_h, c.b_h);
+        TS_SWEEP3(0, 1, c.a_h, c.b_h);
+        TS_SWEEP3(1, 0, c.a_h, c.b_h);
+        TS_SWEEP3(1, 1, c.a_h, c.b_h);
+        TS_SWEEP3(2, 0, c.a_h, c.b_h);
+        if (pot == nullptr) {
+            TS_SWEEP3(2, 1, c.a_f, c.b_f);
+        } else {
+            TS_SWEEP3(2, 1, c.a_h, c.b_h);
+            phase_kernel<T><<<grid_for(sites, 256), 256, 0, st>>>(re, im, pot, pot + sites, sites);
+            ++*launches;
+            TS_CUDA_TRY(cudaGetLastError());
+            TS_SWEEP3(2, 1, c.a_h, c.b_h);
+        }
+        TS_SWEEP3(2, 0, c.a_h, c.b_h);
+        TS_SWEEP3(1, 1, c.a_h, c.b_h);
+        TS_SWEEP3(1, 0, c.a_h, c.b_h);
+        TS_SWEEP3(0, 1, c.a_h, c.b_h);
+        TS_SWEEP3(0, 0, c.a_h, c.b_h);
+    }
+#undef TS_SWEEP3
+    return TS_OK;
+}
+}  // namespace
+
+int generic3_evolve(const Lattice3& L, void* re, void* im, const StepCoef& c, const void* pot,
+                    int64_t n_steps, cudaStream_t st, int64_t* launches) {
+    if (L.dtype == TS_F32)
+        return evolve3_t<float>(L, (float*)re, (float*)im, c, (const float*)pot, n_steps, st, launches);
+    return evolve3_t<double>(L, (double*)re, (double*)im, c, (const double*)pot, n_steps, st, launches);
+}
+
 size_t norm_workspace_doubles() { return kNormBlocks + 1; }
 
 int norm2_device(const LatticeDesc& L, const void* re, const void* im, double* d_work,

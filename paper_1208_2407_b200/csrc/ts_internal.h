@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string>
+#include <vector>
 
 #include "ts.h"
 
@@ -16,6 +17,37 @@ int cuda_fail(cudaError_t e, const char* what);   // records the CUDA string, re
         cudaError_t e_ = (expr);                                      \
         if (e_ != cudaSuccess) return ::ts::cuda_fail(e_, #expr);     \
     } while (0)
+
+// Optional per-launch timing (plan option "timing"): CUDA events around every kernel or copy of
+// one ts_evolve* call, on the launch stream; read back with ts_plan_get_launch_times.
+enum LaunchKind {
+    kKindGeneric = 1,   // the per-sweep kernels of one whole call (not split)
+    kKindFused = 2,     // fused_kernel pass (register prefetch)
+    kKindStream = 3,    // stream_kernel pass (TMA ring)
+    kKindTiny = 4,      // tiny_kernel (whole evolution)
+    kKindLineRows = 5,  // line_kernel along rows (resident lines, all sub-steps)
+    kKindLineCols = 6,  // line_kernel along columns
+    kKindXwin = 7,      // xwin_kernel pass (windowed rows)
+    kKindYcol = 8,      // ycol_kernel pass (pipelined columns)
+    kKindCopy = 9,      // device-to-device copy of a plane
+    kKindExpand = 10,   // separable phase written out as planes
+    kKindLineZ = 11     // line_kernel along z (3-D lattices)
+};
+struct LaunchTimer {
+    struct Rec {
+        int kind;
+        cudaEvent_t a, b;
+    };
+    std::vector<Rec> recs;
+    size_t used = 0;
+    void reset() { used = 0; }
+    void begin(int kind, cudaStream_t st);
+    void end(cudaStream_t st);
+    ~LaunchTimer();
+};
+// null-safe helpers
+inline void timer_begin(LaunchTimer* t, int kind, cudaStream_t st) { if (t) t->begin(kind, st); }
+inline void timer_end(LaunchTimer* t, cudaStream_t st) { if (t) t->end(st); }
 
 // Double-precision description of one step; each path converts to its own arithmetic form.
 struct StepCoef {
@@ -107,6 +139,22 @@ int axis_default_chain(const LatticeDesc& L);
 // chain: sub-steps per windowed / pipelined pass (0 = default); seg_rows, nst: 0 = default.
 int axis_evolve(const LatticeDesc& L, void* psi_re, void* psi_im, void* scr_re, void* scr_im,
                 const StepCoef* pat, int period, int64_t n_sub, int chain, int seg_rows, int nst,
-                cudaStream_t st, AxisInfo* info);
+                cudaStream_t st, AxisInfo* info, LaunchTimer* timer = nullptr);
+
+
+// ---- three-dimensional lattices ------------------------------------------------------------------------
+struct Lattice3 {
+    int64_t nx, ny, nz;
+    int dtype;
+    int per[3];       // periodic flag of the x, y, z axis
+};
+// every axis resident in registers (even extents that fit a thread block), cos of every angle > 0.25
+bool axis3_supported(const Lattice3& L, const StepCoef& c);
+// n_steps steps on psi[nz][ny][nx], in place; pot = null or phase planes [2][nz][ny][nx]
+int axis3_evolve(const Lattice3& L, void* re, void* im, const StepCoef& c, const void* pot,
+                 int64_t n_steps, cudaStream_t st, AxisInfo* info, LaunchTimer* timer);
+// per-sweep kernels (ts_generic.cu): 11 / 13 launches per step, any extents
+int generic3_evolve(const Lattice3& L, void* re, void* im, const StepCoef& c, const void* pot,
+                    int64_t n_steps, cudaStream_t st, int64_t* launches);
 
 }  // namespace ts

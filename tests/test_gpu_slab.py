@@ -34,7 +34,9 @@ def test_per_axis_boundaries(nx, ny, dtype, with_pot, fuse, bx, by):
     re, im, pot = G.random_inputs(nx, ny, dtype, 31 * nx + ny + fuse, with_pot)
     tdt = torch.float32 if dtype == "f32" else torch.float64
     plan = Plan(nx, ny, tdt, bx, by)
-    stream_path = bx == "periodic"       # (closed x, periodic y) runs on the per-sweep kernels
+    # (closed x, periodic y): the axis-split path without a potential (each axis has its own
+    # boundary there), the per-sweep kernels with one
+    stream_path = bx == "periodic"
     if stream_path:
         plan.set_option("path", 2); plan.set_option("variant", 2)
         plan.set_option("fuse_steps", fuse); plan.set_option("seg_rows", 16)
@@ -43,7 +45,11 @@ def test_per_axis_boundaries(nx, ny, dtype, with_pot, fuse, bx, by):
     n = 9
     plan.evolve(dre, dim, *coeffs(0.3), pot_phase=dpot, n_steps=n)
     torch.cuda.synchronize()
-    assert plan.info("fused") == (1 if stream_path else 0)
+    # 128 sites are a resident line of the axis-split path; 380 are neither that nor long enough
+    # for windowed rows
+    axis_path = not stream_path and not with_pot and nx == 128
+    assert plan.info("fused") == (1 if stream_path or axis_path else 0)
+    assert plan.info("variant") == (2 if stream_path else (4 if axis_path else 0))
     wre, wim = re.astype(np.float64), im.astype(np.float64)
     p64 = None if pot is None else (pot[0].astype(np.float64), pot[1].astype(np.float64))
     oracle.evolve_xy(wre, wim, *coeffs(0.3), pot=p64, periodic_x=bx == "periodic",
