@@ -133,6 +133,16 @@ int ts_evolve_u4(ts_plan* plan, void* psi_re, void* psi_im, double theta,
                  int64_t n_steps, void* cuda_stream);
 
 /*
+ * ts_u4_coefficients -- the coefficient table of ONE fourth-order step (Eq. 4), as
+ * ts_evolve_u4 uses it: five rows (a_half, b_half, a_full, b_full) for the sub-step angles
+ * p theta, p theta, (1-4p) theta, p theta, p theta with p = (4 - 4^(1/3))^-1, in order of
+ * application.  For callers that schedule passes themselves (ts_slab_pass): the method's
+ * constants come from the library, not from the binding.  Host arithmetic only; no device needed.
+ *   out20   HOST array of 20 doubles.            Errors: TS_EINVAL (NULL, non-finite theta).
+ */
+int ts_u4_coefficients(double theta, double* out20);
+
+/*
  * ts_evolve_sep -- ts_evolve for a SEPARABLE potential V(x, y) = Vx(x) + Vy(y) (the harmonic trap
  * of the benchmark configs is one): the phase of the diagonal step factorises,
  * exp(-i V dt) = px(x) * py(y), and is passed as two vectors instead of two planes

@@ -15,7 +15,7 @@ _lib = None
 
 SYMBOLS = ["ts_plan_create", "ts_plan_create_xy", "ts_plan_create_3d", "ts_evolve", "ts_evolve_3d", "ts_evolve_u4", "ts_evolve_sep", "ts_evolve_tdep", "ts_slab_pass",
            "ts_norm", "ts_evolve_host", "ts_plan_set_option",
-           "ts_plan_get_info", "ts_plan_reserve", "ts_plan_get_launch_times", "ts_plan_destroy",
+           "ts_plan_get_info", "ts_u4_coefficients", "ts_plan_reserve", "ts_plan_get_launch_times", "ts_plan_destroy",
            "ts_last_error"]
 
 # kinds reported by ts_plan_get_launch_times (include/ts.h)
@@ -67,6 +67,8 @@ def lib():
         L.ts_plan_set_option.restype = i32
         L.ts_plan_get_info.argtypes = [vp, ctypes.c_char_p, ctypes.POINTER(i64)]
         L.ts_plan_get_info.restype = i32
+        L.ts_u4_coefficients.argtypes = [dbl, ctypes.POINTER(dbl)]
+        L.ts_u4_coefficients.restype = i32
         L.ts_plan_reserve.argtypes = [vp, i32]
         L.ts_plan_reserve.restype = i32
         L.ts_plan_get_launch_times.argtypes = [vp, i32, ctypes.POINTER(i32),
@@ -87,6 +89,13 @@ def last_error() -> str:
 def _check(rc):
     if rc != TS_OK:
         raise TsError(rc, last_error())
+
+
+def u4_coefficients(theta: float):
+    """ts_u4_coefficients: the five (a_half, b_half, a_full, b_full) rows of one fourth-order step."""
+    out = (ctypes.c_double * 20)()
+    _check(lib().ts_u4_coefficients(float(theta), out))
+    return [tuple(out[4 * k:4 * k + 4]) for k in range(5)]
 
 
 def _dtype_code(torch_dtype):

@@ -616,18 +616,30 @@ int ts_evolve_tdep(ts_plan* plan, void* psi_re, void* psi_im, double a_half, dou
     return rc;
 }
 
+int ts_u4_coefficients(double theta, double* out20) {
+    if (!out20) return fail(TS_EINVAL, "NULL output table");
+    if (!isfinite(theta)) return fail(TS_EINVAL, "theta must be finite");
+    // Eq. 4 (PAPER.md:93-101): U4(dt) = U2(p dt) U2(p dt) U2((1-4p) dt) U2(p dt) U2(p dt)
+    const double p = 1.0 / (4.0 - cbrt(4.0));
+    const double frac[5] = {p, p, 1.0 - 4.0 * p, p, p};
+    for (int k = 0; k < 5; ++k) {
+        const double th = frac[k] * theta;
+        out20[4 * k] = cos(0.5 * th); out20[4 * k + 1] = sin(0.5 * th);
+        out20[4 * k + 2] = cos(th); out20[4 * k + 3] = sin(th);
+    }
+    return TS_OK;
+}
+
 int ts_evolve_u4(ts_plan* plan, void* psi_re, void* psi_im, double theta, const void* pot_p,
                  const void* pot_q, int64_t n_steps, void* cuda_stream) {
     if ((pot_p == nullptr) != (pot_q == nullptr))
         return fail(TS_EINVAL, "give both potential-phase arrays of the fourth-order step or neither");
     if (!isfinite(theta)) return fail(TS_EINVAL, "theta must be finite");
-    // Eq. 4 (PAPER.md:93-101): U4(dt) = U2(p dt) U2(p dt) U2((1-4p) dt) U2(p dt) U2(p dt)
-    const double p = 1.0 / (4.0 - cbrt(4.0));
-    const double frac[5] = {p, p, 1.0 - 4.0 * p, p, p};
+    double coef[20];
+    ts_u4_coefficients(theta, coef);
     SubStep pat[5];
     for (int k = 0; k < 5; ++k) {
-        const double th = frac[k] * theta;
-        pat[k].c = ts::StepCoef{cos(0.5 * th), sin(0.5 * th), cos(th), sin(th)};
+        pat[k].c = ts::StepCoef{coef[4 * k], coef[4 * k + 1], coef[4 * k + 2], coef[4 * k + 3]};
         const void* pot = k == 2 ? pot_q : pot_p;
         pat[k].ph = ts::Phase{pot ? 1 : 0, pot, nullptr, nullptr};
     }

@@ -38,6 +38,7 @@
 #include <string.h>
 
 #include <atomic>
+#include <vector>
 #include <type_traits>
 
 #include "ts_internal.h"
@@ -332,6 +333,43 @@ __device__ __forceinline__ void phase_mul(Cx<T>& s, T pr, T pi) {
     s.im = fma(m, pr, r * pi);
 }
 
+// Boundary-site exchange between the warps of one line, branch-free: lane 0 / lane 31 store and
+// load their site under a predicate (an `if` around them costs two
+// divergent branches and a reconvergence per sub-step; ncu: branch_resolving was the top stall of
+// the 16-warp kernel).
+__device__ __forceinline__ void st_if(bool pred, uint32_t addr, const Cx<float>& v) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.u32 p, %0, 0;\n\t"
+        "@p st.shared.v2.f32 [%1], {%2, %3};\n\t"
+        "}" ::"r"((uint32_t)pred), "r"(addr), "f"(v.re), "f"(v.im) : "memory");
+}
+__device__ __forceinline__ void st_if(bool pred, uint32_t addr, const Cx<double>& v) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.u32 p, %0, 0;\n\t"
+        "@p st.shared.v2.f64 [%1], {%2, %3};\n\t"
+        "}" ::"r"((uint32_t)pred), "r"(addr), "d"(v.re), "d"(v.im) : "memory");
+}
+__device__ __forceinline__ void ld_if(bool pred, uint32_t addr, Cx<float>& v) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.u32 p, %2, 0;\n\t"
+        "@p ld.shared.v2.f32 {%0, %1}, [%3];\n\t"
+        "}" : "+f"(v.re), "+f"(v.im) : "r"((uint32_t)pred), "r"(addr) : "memory");
+}
+__device__ __forceinline__ void ld_if(bool pred, uint32_t addr, Cx<double>& v) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.u32 p, %2, 0;\n\t"
+        "@p ld.shared.v2.f64 {%0, %1}, [%3];\n\t"
+        "}" : "+d"(v.re), "+d"(v.im) : "r"((uint32_t)pred), "r"(addr) : "memory");
+}
+
 // COL = false: rows (site stride 1, 16-byte accesses); COL = true: columns (site stride = pitch,
 // scalar accesses; the warps of a block take adjacent columns at the same time, so that the
 // 32-byte sectors they share are fetched once).  MW = false: one warp per line, nothing but
@@ -357,6 +395,15 @@ line_kernel(const __grid_constant__ LineParams<T> p) {
     }
     const uint32_t bar = smem_u32(&xbar[MW ? grp : 0]);
     uint32_t ph = 0, par = 0;
+    // xbuf[line][parity set][b] = {first site of warp b, last site of warp b - 1}: the two sites of
+    // the pair that straddles warps b - 1 and b, next to each other.  Lane 0 of warp b writes
+    // entry b's first half and reads its second; lane 31 of warp b - 1 the other way round -- one
+    // store address and one load address per lane (parity set 1 is kParB further on).
+    constexpr uint32_t kParB = (MW ? kMaxLineWarps : 1) * 2 * sizeof(Cx<T>);
+    const bool is_first = lane == 0, is_last = lane == 31;
+    const int bnd = is_last ? (wl == W - 1 ? 0 : wl + 1) : wl;
+    const uint32_t xb_st = smem_u32(&xbuf[grp][0][MW ? bnd : 0][is_last ? 1 : 0]);
+    const uint32_t xb_ld = smem_u32(&xbuf[grp][0][MW ? bnd : 0][is_last ? 0 : 1]);
 
     const int xl = (wl * 32 + lane) * NS;       // first site of the lane
     const bool active = MW || lane < p.n_lanes;
@@ -403,10 +450,10 @@ line_kernel(const __grid_constant__ LineParams<T> p) {
             if (MW) {
                 // publish the boundary sites (state after the even sweep); the wait for the
                 // neighbouring warps' comes after the in-thread work
-                if (lane == 0) xbuf[grp][par][wl][0] = M.s[0];
-                if (lane == 31) xbuf[grp][par][wl][1] = M.s[NS - 1];
+                st_if(is_first, xb_st + par, M.s[0]);
+                st_if(is_last, xb_st + par, M.s[NS - 1]);
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar);
+                if (is_first) mbar_arrive(bar);
             }
             up.re = __shfl_sync(0xffffffffu, M.s[NS - 1].re, up_src);
             up.im = __shfl_sync(0xffffffffu, M.s[NS - 1].im, up_src);
@@ -417,10 +464,9 @@ line_kernel(const __grid_constant__ LineParams<T> p) {
             if (MW) {
                 mbar_wait(bar, ph);
                 ph ^= 1;
-                const int wu = wl == 0 ? W - 1 : wl - 1, wd = wl == W - 1 ? 0 : wl + 1;
-                if (lane == 0) up = xbuf[grp][par][wu][1];
-                if (lane == 31) dn = xbuf[grp][par][wd][0];
-                par ^= 1;
+                ld_if(is_first, xb_ld + par, up);
+                ld_if(is_last, xb_ld + par, dn);
+                par ^= kParB;
             }
         };
         if (p.n_prog == 0) {
@@ -980,8 +1026,10 @@ LineGeom cols_of(const LatticeDesc& L) {
 // launch the line kernel on lines held completely in registers; p carries a chain (fill_chain) or
 // a sweep program (fill_prog)
 template <typename T>
-int launch_lines(const LineGeom& g, int dtype, LineParams<T>& p, T* re, T* im, cudaStream_t st) {
-    p.src_re = re; p.src_im = im; p.dst_re = re; p.dst_im = im;
+int launch_lines(const LineGeom& g, int dtype, LineParams<T>& p, T* re, T* im, cudaStream_t st,
+                 T* out_re = nullptr, T* out_im = nullptr) {
+    p.src_re = re; p.src_im = im;
+    p.dst_re = out_re ? out_re : re; p.dst_im = out_im ? out_im : im;
     p.n_lines = (int)g.n_lines;
     p.n_sites = (int)g.n_sites;
     p.line_stride = g.line_stride;
@@ -1010,10 +1058,10 @@ int launch_lines(const LineGeom& g, int dtype, LineParams<T>& p, T* re, T* im, c
 // or the columns, in place.
 template <typename T>
 int line_pass(const LatticeDesc& L, T* re, T* im, const StepCoef* pat, int period, int64_t n_sub,
-              bool col, cudaStream_t st) {
+              bool col, cudaStream_t st, T* out_re = nullptr, T* out_im = nullptr) {
     LineParams<T> p = {};
     fill_chain(p, pat, period, 0, n_sub, col);
-    return launch_lines<T>(col ? cols_of(L) : rows_of(L), L.dtype, p, re, im, st);
+    return launch_lines<T>(col ? cols_of(L) : rows_of(L), L.dtype, p, re, im, st, out_re, out_im);
 }
 
 // Constants of a sweep program: sweeps (parity, angle) applied in order, scales followed as in
@@ -1253,18 +1301,59 @@ static int axis_evolve_t(const LatticeDesc& L, T* psi_re, T* psi_im, T* scr_re, 
     const bool x_res = line_shape(L.nx, L.dtype).ok();
     const bool y_res = column_resident(L);
     int rc;
+    // ---- the windowed / pipelined passes of this call (out of place, ping-pong)
+    struct Pass { int s, S; };
+    std::vector<Pass> ypasses;
+    int x_chain = 0;
+    int64_t n_xpass = 0;
+    if (!x_res) {
+        x_chain = chain < kMaxChain ? chain : kMaxChain;
+        n_xpass = (n_sub + x_chain - 1) / x_chain;
+    }
+    if (!y_res) {
+        const int smax = ycol_depth(kMaxChain, L.dtype);
+        int want = (int)(n_sub < chain ? n_sub : chain);
+        if (want > smax) want = smax;
+        for (int64_t i = 0; i < n_sub;) {
+            Pass ps;
+            if (period == 1) {
+                // uniform steps: passes of exactly an instantiated depth run on the kernel whose
+                // coefficients stay in uniform registers (200 = 8 x 24 + 8); what is left below
+                // the smallest depth is one padded pass
+                const int64_t left = n_sub - i;
+                const int cap = (int)(left < want ? left : want);
+                ps.S = ycol_depth(cap, L.dtype);
+                if (ps.S > cap && cap >= 4) ps.S = cap / 4 * 4;       // depths are the multiples of 4
+                ps.s = ps.S < cap ? ps.S : cap;
+            } else {
+                // equal passes: 200 sub-steps at depth 24 are 9 passes of 22 or 23
+                const int64_t n_pass = (n_sub + want - 1) / want;
+                const int per_pass = (int)((n_sub + n_pass - 1) / n_pass);
+                ps.S = ycol_depth(per_pass, L.dtype);
+                ps.s = (int)(n_sub - i < per_pass ? n_sub - i : per_pass);
+            }
+            ypasses.push_back(ps);
+            i += ps.s;
+        }
+    }
+    // a resident-line launch works in place or, for free, into the other buffer: it takes the odd
+    // flip when the out-of-place passes are odd in number, so that the result lands in the caller's
+    // planes without a final copy
+    const bool odd_flips = ((n_xpass + (int64_t)ypasses.size()) & 1) != 0;
     // ---- rows
     if (x_res) {
+        const bool flip_here = odd_flips;
         timer_begin(tm, kKindLineRows, st);
-        rc = line_pass<T>(L, cur_re, cur_im, pat, period, n_sub, false, st);
+        rc = line_pass<T>(L, cur_re, cur_im, pat, period, n_sub, false, st,
+                          flip_here ? nxt_re : nullptr, flip_here ? nxt_im : nullptr);
         timer_end(tm, st);
         if (rc != TS_OK) return rc;
+        if (flip_here) flip();
         ++info->passes; ++info->launches;
         info->chain_x = n_sub;
     } else {
-        const int sx = chain < kMaxChain ? chain : kMaxChain;
-        for (int64_t i = 0; i < n_sub; i += sx) {
-            const int64_t s = n_sub - i < sx ? n_sub - i : sx;
+        for (int64_t i = 0; i < n_sub; i += x_chain) {
+            const int64_t s = n_sub - i < x_chain ? n_sub - i : x_chain;
             timer_begin(tm, kKindXwin, st);
             rc = xwin_pass<T>(L, cur_re, cur_im, nxt_re, nxt_im, pat, period, i, s, st);
             timer_end(tm, st);
@@ -1272,20 +1361,20 @@ static int axis_evolve_t(const LatticeDesc& L, T* psi_re, T* psi_im, T* scr_re, 
             flip();
             ++info->passes; ++info->launches;
         }
-        info->chain_x = sx;
+        info->chain_x = x_chain;
     }
     // ---- columns
     if (y_res) {
+        const bool flip_here = odd_flips && !x_res;
         timer_begin(tm, kKindLineCols, st);
-        rc = line_pass<T>(L, cur_re, cur_im, pat, period, n_sub, true, st);
+        rc = line_pass<T>(L, cur_re, cur_im, pat, period, n_sub, true, st,
+                          flip_here ? nxt_re : nullptr, flip_here ? nxt_im : nullptr);
         timer_end(tm, st);
         if (rc != TS_OK) return rc;
+        if (flip_here) flip();
         ++info->passes; ++info->launches;
         info->chain_y = n_sub;
     } else {
-        const int smax = ycol_depth(kMaxChain, L.dtype);
-        int want = (int)(n_sub < chain ? n_sub : chain);
-        if (want > smax) want = smax;
         // ring slots per warp: at least 3 (iteration i+2 is waited for while slot i-1 is the one
         // being refilled), at most what 200 KB of shared memory per block hold
         int slots = nst >= 3 ? nst : (nst > 0 ? 3 : 8);
@@ -1293,24 +1382,8 @@ static int axis_evolve_t(const LatticeDesc& L, T* psi_re, T* psi_im, T* scr_re, 
         if (slots > slot_max) slots = slot_max;
         StepCoef subs[kMaxChain];
         int64_t i = 0;
-        while (i < n_sub) {
-            int s, S;
-            if (period == 1) {
-                // uniform steps: passes of exactly an instantiated depth run on the kernel whose
-                // coefficients stay in uniform registers (200 = 8 x 24 + 8); what is left below
-                // the smallest depth is one padded pass
-                const int64_t left = n_sub - i;
-                const int cap = (int)(left < want ? left : want);
-                S = ycol_depth(cap, L.dtype);
-                if (S > cap && cap >= 4) S = cap / 4 * 4;       // depths are the multiples of 4
-                s = S < cap ? S : cap;
-            } else {
-                // equal passes: 200 sub-steps at depth 24 are 9 passes of 22 or 23
-                const int64_t n_pass = (n_sub + want - 1) / want;
-                const int per_pass = (int)((n_sub + n_pass - 1) / n_pass);
-                S = ycol_depth(per_pass, L.dtype);
-                s = (int)(n_sub - i < per_pass ? n_sub - i : per_pass);
-            }
+        for (size_t k = 0; k < ypasses.size(); ++k) {
+            const int s = ypasses[k].s, S = ypasses[k].S;
             for (int j = 0; j < s; ++j) subs[j] = pat[(i + j) % period];
             const bool uni = period == 1 && s == S && S > 1;
             const int seg = seg_rows > 0 ? seg_rows : ycol_default_seg(L, S, uni);
@@ -1320,7 +1393,7 @@ static int axis_evolve_t(const LatticeDesc& L, T* psi_re, T* psi_im, T* scr_re, 
             if (rc != TS_OK) return rc;
             flip();
             ++info->passes; ++info->launches;
-            if (i == 0) { info->chain_y = s; info->seg_rows = seg; }
+            if (k == 0) { info->chain_y = s; info->seg_rows = seg; }
             i += s;
         }
     }

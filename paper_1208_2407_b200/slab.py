@@ -289,16 +289,11 @@ def max_fused_steps(dtype, with_pot: bool = False) -> int:
     return 6 if (dtype == torch.float32 and not with_pot) else 4
 
 
-def step_coeffs(theta):
-    """(a_half, b_half, a_full, b_full) of one second-order step of angle theta."""
-    import math
-    return (math.cos(theta / 2), math.sin(theta / 2), math.cos(theta), math.sin(theta))
-
-
 def u4_pattern(theta):
-    """The five sub-steps of the fourth-order step, Eq. 4."""
-    p = 1.0 / (4.0 - 4.0 ** (1.0 / 3.0))
-    return [step_coeffs(f * theta) for f in (p, p, 1.0 - 4.0 * p, p, p)]
+    """The five sub-steps of the fourth-order step, Eq. 4: the library's table
+    (ts_u4_coefficients) -- the binding holds none of the method's arithmetic."""
+    from .binding import u4_coefficients
+    return u4_coefficients(theta)
 
 
 def _passes(pattern, n_repeat, depth):
@@ -317,9 +312,9 @@ class PeerSlab:
     straight from the neighbours' source buffers (same GPU here, a peer GPU's mapped memory in
     `PeerRank`).  buffers: optional [2][2][rows >= own][nx] tensor to live in (symmetric memory)."""
 
-    def __init__(self, nx, ny, dtype, boundary, rank, world, device, buffers=None):
+    def __init__(self, nx, ny, dtype, boundary, rank, world, device, buffers=None, pass_fn=None,
+                 norm_fn=None):
         import torch
-        from .binding import Plan
         self.nx, self.ny, self.dtype, self.boundary = int(nx), int(ny), dtype, boundary
         self.rank, self.world = int(rank), int(world)
         self.r0, self.r1 = partition_rows(self.ny, self.world)[self.rank]
@@ -333,7 +328,12 @@ class PeerSlab:
         self.buffers = buffers
         self.cur = 0
         self.sep = None
-        self.plan = Plan(self.nx, self.own, dtype, boundary, "closed")
+        # pass_fn / norm_fn stand in for ts_slab_pass / ts_norm in the CPU tests of the sequencing
+        self.pass_fn, self.norm_fn = pass_fn, norm_fn
+        self.plan = None
+        if pass_fn is None:
+            from .binding import Plan
+            self.plan = Plan(self.nx, self.own, dtype, boundary, "closed")
         self.norm_plan = self.plan
 
     def planes(self, which):
@@ -353,6 +353,9 @@ class PeerSlab:
         """dst <- U2(subs[-1]) ... U2(subs[0]) src with the neighbours' CURRENT planes as halos;
         does not flip."""
         px, py = self.sep if self.sep is not None else (None, None)
+        if self.pass_fn is not None:
+            self.pass_fn(self, self.planes(self.cur), self.planes(1 - self.cur), up_src, dn_src, subs)
+            return
         self.plan.slab_pass(self.planes(self.cur), self.planes(1 - self.cur), up_src, dn_src,
                             subs, px, py, self.r0, self.ny, self.boundary == "periodic",
                             stream=stream)
@@ -362,10 +365,27 @@ class PeerSlab:
 
     def norm_local(self) -> float:
         re, im = self.planes(self.cur)
+        if self.norm_fn is not None:
+            return self.norm_fn(re, im)
         return self.plan.norm(re, im)
 
     def destroy(self):
-        self.plan.destroy()
+        if self.plan is not None:
+            self.plan.destroy()
+
+
+class SymmetricMemory:
+    """Where PeerRank's buffers live: torch.distributed._symmetric_memory (CUDA, one process per
+    GPU).  alloc -> a tensor every peer can map; rendezvous -> a handle with get_buffer(rank, shape,
+    dtype, offset) and barrier(channel).  The CPU tests pass a stand-in with the same two calls."""
+
+    def alloc(self, shape, dtype, device):
+        import torch.distributed._symmetric_memory as symm
+        return symm.empty(shape, dtype=dtype, device=device)
+
+    def rendezvous(self, buf, group):
+        import torch.distributed._symmetric_memory as symm
+        return symm.rendezvous(buf, group)
 
 
 class PeerGroup:
@@ -432,19 +452,21 @@ class PeerRank:
     pass k".  NOT RUN on hardware in this round (needs >= 2 GPUs); the single-process twin
     `PeerGroup` runs the identical kernel path with neighbours on the same device."""
 
-    def __init__(self, nx, ny, dtype, boundary, group=None):
+    def __init__(self, nx, ny, dtype, boundary, group=None, memory=None, device=None, pass_fn=None,
+                 norm_fn=None):
         import torch
         import torch.distributed as dist
-        import torch.distributed._symmetric_memory as symm
         self.group = group if group is not None else dist.group.WORLD
         rank, world = dist.get_rank(self.group), dist.get_world_size(self.group)
-        dev = torch.device("cuda", torch.cuda.current_device())
+        dev = device if device is not None else torch.device("cuda", torch.cuda.current_device())
+        memory = memory if memory is not None else SymmetricMemory()
         rows = max(b - a for a, b in partition_rows(ny, world))      # same shape on every rank
         self.shape = (2, 2, rows, int(nx))
-        buf = symm.empty(self.shape, dtype=dtype, device=dev)
+        buf = memory.alloc(self.shape, dtype, dev)
         buf.zero_()
-        self.handle = symm.rendezvous(buf, self.group)
-        self.slab = PeerSlab(nx, ny, dtype, boundary, rank, world, dev, buffers=buf)
+        self.handle = memory.rendezvous(buf, self.group)
+        self.slab = PeerSlab(nx, ny, dtype, boundary, rank, world, dev, buffers=buf, pass_fn=pass_fn,
+                             norm_fn=norm_fn)
         parts = partition_rows(ny, world)
         self.peer_own = [b - a for a, b in parts]
         self.peer_buf = {}
@@ -466,12 +488,20 @@ class PeerRank:
         n = self.peer_own[r]
         return b[0, :n], b[1, :n]
 
-    def run(self, pattern, n_repeat):
+    def run(self, pattern, n_repeat, stream=None):
+        """One barrier per pass: it orders "every rank has written pass k-1" before "anybody reads
+        it" (RAW) and, because a rank reaches barrier k+1 only after its own pass k, also "every
+        neighbour has read my pass k-1 source" before pass k+1 overwrites it (WAR).  The barrier
+        and the pass must be enqueued on the SAME stream (torch's current one by default)."""
+        import torch
         s = self.slab
+        if stream is not None and s.plan is not None:
+            assert stream.cuda_stream == torch.cuda.current_stream().cuda_stream, \
+                "PeerRank: handle.barrier runs on the current stream; launch the passes there too"
         for subs in _passes(pattern, n_repeat, self.S):
             self.handle.barrier(channel=0)          # every rank's previous pass is complete
             s.launch_pass(self._peer_planes(s.nb.up, s.cur), self._peer_planes(s.nb.down, s.cur),
-                          subs)
+                          subs, stream=stream)
             s.flip()                                # all ranks flip in step: same parity everywhere
         self.handle.barrier(channel=0)
 

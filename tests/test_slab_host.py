@@ -103,4 +103,4 @@ def test_pass_cutting_and_u4_pattern():
     assert [len(p) for p in passes] == [6, 6, 6, 2]
     flat = [c for p in passes for c in p]
     assert flat == pat * 4
-    assert list(slab._passes([slab.step_coeffs(0.1)], 0, 6)) == []
+    assert list(slab._passes([(1.0, 0.0, 1.0, 0.0)], 0, 6)) == []
