@@ -121,8 +121,10 @@ def oracle_sample(cfg_name, budget_site_steps, full_ok=False):
     cfg = inputs.CONFIGS[cfg_name]
     need = cfg.sites * 8 * (2 + (2 if cfg.has_pot else 0)) * 2.5      # float64 planes + generation
     ram = host_ram_bytes()
-    if cfg.sites <= budget_site_steps and (cfg.sites <= 2 ** 24 or (full_ok and need < 0.5 * ram)):
+    if cfg.sites <= 2 ** 24 and cfg.sites <= budget_site_steps:                      # C1 - C3
         return cfg, max(1, min(cfg.n_steps, int(budget_site_steps // cfg.sites)))
+    if full_ok and cfg.sites <= 2 ** 28 and 2 * cfg.sites <= budget_site_steps and need < 0.5 * ram:
+        return cfg, 2                                                                # C4: 2 steps
     n = min(cfg.nx, 2048)
     small = inputs.scaled(cfg, n, n)
     steps = max(1, min(cfg.n_steps, int(budget_site_steps // small.sites)))
@@ -470,6 +472,93 @@ def run_gpu(args):
     return 0
 
 
+def run_gpu_3d(args):
+    """--lattice3d N: an N^3 fp32 lattice (the 3-D extension), periodic, seeded
+    uniform state as in C4, theta = 0.02, 100 second-order steps per ts_evolve_3d call; with
+    --pot3d a seeded random phase field.  Not one of BASELINE.json's configs: a bench line for the
+    SURVEY 8(f) NEXT-4 row, same metric."""
+    import torch
+    from paper_1208_2407_b200.binding import Plan3D, LAUNCH_KINDS
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    n, n_steps, theta = args.lattice3d, 100, 0.02
+    if args.pot3d:
+        n_steps = 20
+    g = torch.Generator(device=dev); g.manual_seed(12082407)
+    re = torch.rand((n, n, n), device=dev, generator=g) * 2 - 1
+    im = torch.rand((n, n, n), device=dev, generator=g) * 2 - 1
+    nrm = float(torch.sqrt((re.double() ** 2 + im.double() ** 2).sum()))
+    re /= nrm; im /= nrm
+    pot = None
+    if args.pot3d:
+        V = torch.rand((n, n, n), device=dev, generator=g, dtype=torch.float64) * 6.28
+        pot = torch.stack([torch.cos(V), -torch.sin(V)]).float().contiguous()
+        del V
+    plan = Plan3D(n, n, n, torch.float32, "periodic")
+    c = (math.cos(theta / 2), math.sin(theta / 2), math.cos(theta), math.sin(theta))
+    stream = torch.cuda.current_stream()
+    call = lambda: plan.evolve(re, im, *c, pot_phase=pot, n_steps=n_steps, stream=stream)
+    n0 = plan.norm(re, im)
+    for _ in range(args.warmup):
+        call()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start(); time.sleep(0.25)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.time()
+    e0.record(stream)
+    for _ in range(args.steps):
+        call()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    t1 = time.time()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop(t0, t1)
+    n1 = plan.norm(re, im)
+    plan.set_option("timing", 1)
+    call(); torch.cuda.synchronize()
+    per_kind = {}
+    for kind, kms in plan.launch_times():
+        per_kind.setdefault(kind, []).append(kms)
+    plan.set_option("timing", 0)
+    sites = n ** 3
+    peak, peak_src = load_peaks()
+    alu = ALU_PEAK_TFLOPS["f32"]
+    kernels = []
+    for k, v in sorted(per_kind.items(), key=lambda kv: -sum(kv[1])):
+        by = sites * (16 + (8 if (pot is not None and k == 11) else 0))
+        fl = sites * 8 * n_steps if pot is None else sites * (12 + (6 if k == 11 else 0))
+        avg = sum(v) / len(v)
+        kernels.append({"kernel": LAUNCH_KINDS.get(k, str(k)), "launches_per_call": len(v),
+                        "avg_ms": avg, "hbm_frac": by / (peak * 1e9) * 1e3 / avg,
+                        "alu_frac": fl / (alu * 1e12) * 1e3 / avg})
+    top = kernels[0]
+    bound = "alu" if top["alu_frac"] > top["hbm_frac"] else "hbm"
+    line = {
+        "metric": METRIC, "value": sites * n_steps * args.steps / (ms * 1e-3), "unit": UNIT,
+        "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": f"3-D {n}^3 f32 periodic, {'random phase field' if pot is not None else 'no potential'}, "
+                               f"theta={theta}, {n_steps} second-order steps per ts_evolve_3d call",
+                   "variant": plan.info("variant"), "launches_per_call": plan.info("launches"),
+                   "norm2_before": n0, "norm_drift": n1 / n0 - 1,
+                   "l2": "state far larger than the 126 MB L2; no flush" if sites * 8 > 2.5e8 else
+                         "state comparable to the 126 MB L2"},
+        "clocks": clocks, "gpu_launches": plan.info("launches") * args.steps,
+        "roofline": {"bound": bound, "frac": top["alu_frac"] if bound == "alu" else top["hbm_frac"],
+                     "peak": alu if bound == "alu" else peak,
+                     "unit": "TFLOP/s" if bound == "alu" else "GB/s",
+                     "achieved": (top["alu_frac"] * alu) if bound == "alu" else top["hbm_frac"] * peak,
+                     "traffic": None, "kernel": top["kernel"], "kernels": kernels,
+                     "peak_source": peak_src},
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def run_gpu_slab(args):
     """ONE lattice cut into row slabs (paper_1208_2407_b200/slab.py): with N > 1 ranks the global
     lattice is nx x (ny * N) (weak scaling: every rank owns a slab of the config's size) and halos
@@ -486,6 +575,11 @@ def run_gpu_slab(args):
     dev = torch.device("cuda", local)
     dist = None
     if world > 1:
+        # the communicator lines (ranks, rings / NVLS, peer access) go to stderr, so that a scaling
+        # run can be checked; stdout stays the one JSON line
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+        os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
     cfg = inputs.CONFIGS[args.config]
@@ -617,6 +711,8 @@ def main():
     ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--fuse-steps", type=int, default=0)
     ap.add_argument("--seg-rows", type=int, default=0)
+    ap.add_argument("--lattice3d", type=int, default=0, help="bench an N^3 fp32 lattice (ts_evolve_3d)")
+    ap.add_argument("--pot3d", action="store_true", help="with --lattice3d: a phase field")
     ap.add_argument("--chain", type=int, default=0, help="axis-split path: sub-steps per pass")
     ap.add_argument("--variant", type=int, default=0, help="plan option variant (0 = default path)")
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
@@ -637,6 +733,8 @@ def main():
         args.warmup = 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.lattice3d:
+        return run_gpu_3d(args)
     if args.decomp == "slab" or args.slabs > 1 or args.slab_mode == "peer":
         return run_gpu_slab(args)
     return run_gpu(args)

@@ -353,6 +353,20 @@ __device__ __forceinline__ void st_if(bool pred, uint32_t addr, const Cx<double>
         "@p st.shared.v2.f64 [%1], {%2, %3};\n\t"
         "}" ::"r"((uint32_t)pred), "r"(addr), "d"(v.re), "d"(v.im) : "memory");
 }
+// wait with a bound: a protocol error traps instead of hanging the device
+__device__ __forceinline__ void mbar_wait_bounded(uint32_t bar, uint32_t parity) {
+    uint32_t done = 0, spins = 0;
+    while (true) {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}" : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        if (done) break;
+        if (++spins > (1u << 24)) __trap();
+    }
+}
 __device__ __forceinline__ void ld_if(bool pred, uint32_t addr, Cx<float>& v) {
     asm volatile(
         "{\n\t"
@@ -379,8 +393,13 @@ template <typename T, int NS, bool EDGE, bool COL, bool MW>
 __global__ void __launch_bounds__(MW ? 512 : 128, MW ? 1 : (sizeof(T) * NS >= 128 ? 3 : 4))
 line_kernel(const __grid_constant__ LineParams<T> p) {
     constexpr int PW = (Piece<T>::n < NS) ? Piece<T>::n : NS;     // sites per vector access
-    // per line: an mbarrier and two (parity) sets of per-warp boundary sites {first, last}
-    __shared__ __align__(16) Cx<T> xbuf[MW ? kMaxLineWarps : 1][2][MW ? kMaxLineWarps : 1][2];
+    // Exchange of the pair that straddles two warps of a line: entry b (b = the block's warp index
+    // of the warp AFTER the cut) holds {first site of warp b, last site of warp b - 1}, twice
+    // (parity sets used by alternate sub-steps), and the line has ONE mbarrier that every warp
+    // arrives on after publishing.  (Measured alternative, r2g: neighbour-to-neighbour barriers --
+    // two arrivals and two waits per warp and sub-step, warps free to drift apart by a sub-step --
+    // C4 rows 10.97 ms against 9.22 ms with the line-wide barrier.)
+    __shared__ __align__(16) Cx<T> xbuf[2][MW ? kMaxLineWarps : 1][2];
     __shared__ __align__(8) uint64_t xbar[MW ? kMaxLineWarps : 1];
 
     const int lane = threadIdx.x & 31;
@@ -395,15 +414,14 @@ line_kernel(const __grid_constant__ LineParams<T> p) {
     }
     const uint32_t bar = smem_u32(&xbar[MW ? grp : 0]);
     uint32_t ph = 0, par = 0;
-    // xbuf[line][parity set][b] = {first site of warp b, last site of warp b - 1}: the two sites of
-    // the pair that straddles warps b - 1 and b, next to each other.  Lane 0 of warp b writes
-    // entry b's first half and reads its second; lane 31 of warp b - 1 the other way round -- one
-    // store address and one load address per lane (parity set 1 is kParB further on).
     constexpr uint32_t kParB = (MW ? kMaxLineWarps : 1) * 2 * sizeof(Cx<T>);
     const bool is_first = lane == 0, is_last = lane == 31;
-    const int bnd = is_last ? (wl == W - 1 ? 0 : wl + 1) : wl;
-    const uint32_t xb_st = smem_u32(&xbuf[grp][0][MW ? bnd : 0][is_last ? 1 : 0]);
-    const uint32_t xb_ld = smem_u32(&xbuf[grp][0][MW ? bnd : 0][is_last ? 0 : 1]);
+    const int w_dn = MW ? grp * W + (wl == W - 1 ? 0 : wl + 1) : 0;     // entry after this warp
+    const int w_me = MW ? grp * W + wl : 0;                             // entry before this warp
+    const int bnd = is_last ? w_dn : w_me;
+    // lane 0 writes its entry's first half and reads the second; lane 31 the other way round
+    const uint32_t xb_st = smem_u32(&xbuf[0][bnd][is_last ? 1 : 0]);
+    const uint32_t xb_ld = smem_u32(&xbuf[0][bnd][is_last ? 0 : 1]);
 
     const int xl = (wl * 32 + lane) * NS;       // first site of the lane
     const bool active = MW || lane < p.n_lanes;
@@ -462,7 +480,7 @@ line_kernel(const __grid_constant__ LineParams<T> p) {
         };
         auto xend = [&](Cx<T>& up, Cx<T>& dn) {
             if (MW) {
-                mbar_wait(bar, ph);
+                mbar_wait_bounded(bar, ph);
                 ph ^= 1;
                 ld_if(is_first, xb_ld + par, up);
                 ld_if(is_last, xb_ld + par, dn);
@@ -511,6 +529,98 @@ line_kernel(const __grid_constant__ LineParams<T> p) {
                 st_piece(p.dst_re + base + xl + k, r, PW);
                 st_piece(p.dst_im + base + xl + k, i, PW);
             }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// strided lines, transposed: one LANE per line
+// ---------------------------------------------------------------------------------------------
+// Lines whose sites are far apart in memory (y and z of a 3-D lattice: stride nx, nx * ny) but
+// whose NEIGHBOURING lines are adjacent: a warp takes 32 adjacent lines, one per lane, so every
+// access is a coalesced 128-byte (fp32) row of 32 lines.  The line itself is cut over the W warps
+// of the block: thread (warp w, lane l) holds sites [w NS, (w+1) NS) of line l -- all pairs are
+// in-thread except the one that straddles two warps, which all 32 lanes exchange through shared
+// memory (one mbarrier per block as in line_kernel, no shuffles at all).  The resident
+// kernel above with strided scalar accesses (COL) touches a different DRAM page with every lane:
+// 512^3 fp32, z lines: 7.5 ms per 100-step chain there, and 13.9 ms per 3-sweep launch with a
+// potential (0.04 of the HBM roofline).
+constexpr int kTWarps = 16;
+template <typename T, int NS, bool EDGE>
+__global__ void __launch_bounds__(kTWarps * 32, 1)
+tline_kernel(const __grid_constant__ LineParams<T> p) {
+    __shared__ __align__(16) Cx<T> xbuf[2][kTWarps][2][32];
+    __shared__ __align__(8) uint64_t xbar;
+    const int lane = threadIdx.x & 31;
+    const int w = threadIdx.x >> 5;
+    const int W = p.n_warps;
+    if (threadIdx.x == 0) mbar_init(smem_u32(&xbar), W);
+    mbar_fence_init();
+    __syncthreads();
+    const uint32_t bar = smem_u32(&xbar);
+    uint32_t ph = 0;
+    int par = 0;
+    const int wu = w == 0 ? W - 1 : w - 1, wd = w == W - 1 ? 0 : w + 1;
+    const bool cut_up = EDGE && !p.periodic && w == 0;
+    const bool cut_dn = EDGE && !p.periodic && w == W - 1;
+    const bool leader = lane == 0;
+
+    for (int64_t l0 = (int64_t)blockIdx.x * 32; l0 < p.n_lines; l0 += (int64_t)gridDim.x * 32) {
+        const int64_t line = l0 + lane;
+        const bool active = line < p.n_lines;
+        const int64_t li = active ? line : p.n_lines - 1;
+        const int64_t g = li / p.lines_inner;
+        const int64_t base = g * p.group_stride + (li - g * p.lines_inner) * p.line_stride +
+                             (int64_t)(w * NS) * p.site_stride;
+        Line<T, NS> L;
+        {   // running pointers: NS precomputed 64-bit offsets would cost 2 NS registers
+            const T* q_re = p.src_re + base;
+            const T* q_im = p.src_im + base;
+#pragma unroll
+            for (int k = 0; k < NS; ++k) {
+                L.s[k].re = active ? __ldg(q_re) : T(0);
+                L.s[k].im = active ? __ldg(q_im) : T(0);
+                q_re += p.site_stride; q_im += p.site_stride;
+            }
+        }
+        auto xbegin = [&](Line<T, NS>& M, Cx<T>& up, Cx<T>& dn) {
+            if (W == 1) { up = M.s[NS - 1]; dn = M.s[0]; return; }     // the line closes on itself
+            xbuf[par][w][0][lane] = M.s[0];
+            xbuf[par][w][1][lane] = M.s[NS - 1];
+            __syncwarp();
+            if (leader) mbar_arrive(bar);
+        };
+        auto xend = [&](Cx<T>& up, Cx<T>& dn) {
+            if (W == 1) return;
+            mbar_wait_bounded(bar, ph);
+            ph ^= 1;
+            up = xbuf[par][wu][1][lane];
+            dn = xbuf[par][wd][0][lane];
+            par ^= 1;
+        };
+        if (p.n_prog == 0) {
+            run_chain<T, NS, EDGE>(p, L, cut_up, cut_dn, xbegin, xend);
+        } else {
+            run_prog<T, NS, EDGE>(p, L, cut_up, cut_dn, xbegin, xend);
+            if (p.ph_re != nullptr && active) {
+                const T* q_re = p.ph_re + base;
+                const T* q_im = p.ph_im + base;
+#pragma unroll
+                for (int k = 0; k < NS; ++k) {
+                    phase_mul(L.s[k], __ldg(q_re), __ldg(q_im));
+                    q_re += p.site_stride; q_im += p.site_stride;
+                }
+            }
+            line_scale2(L, p.fin_e, p.fin_o);
+        }
+        if (!active) continue;
+        T* o_re = p.dst_re + base;
+        T* o_im = p.dst_im + base;
+#pragma unroll
+        for (int k = 0; k < NS; ++k) {
+            *o_re = L.s[k].re;
+            *o_im = L.s[k].im;
+            o_re += p.site_stride; o_im += p.site_stride;
         }
     }
 }
@@ -1008,6 +1118,42 @@ int launch_line_t(const LineParams<T>& p, int ns, bool edge, bool col, cudaStrea
     return TS_EUNSUPPORTED;
 }
 
+// transposed strided lines: n = W * NS, W <= 16 warps; the largest W (most parallelism per line,
+// fewest registers per thread)
+struct TShape {
+    int ns, warps;
+    bool ok() const { return ns != 0; }
+};
+TShape tline_shape(int64_t n, int dtype) {
+    const int ns_max = dtype == TS_F32 ? 32 : 16;
+    for (int ns = 2; ns <= ns_max; ns *= 2)
+        if (n % ns == 0 && n / ns <= kTWarps) return {ns, (int)(n / ns)};
+    return {0, 0};
+}
+template <typename T, int NS>
+int launch_tline_ns(const LineParams<T>& p, bool edge, cudaStream_t st) {
+    const int64_t groups = ((int64_t)p.n_lines + 31) / 32;
+    const int64_t resident = (int64_t)sm_count() * ((kTWarps * 32) / (p.n_warps * 32));
+    const unsigned blocks = (unsigned)(groups < resident ? groups : resident);
+    if (edge) tline_kernel<T, NS, true><<<blocks, p.n_warps * 32, 0, st>>>(p);
+    else tline_kernel<T, NS, false><<<blocks, p.n_warps * 32, 0, st>>>(p);
+    TS_CUDA_TRY(cudaGetLastError());
+    return TS_OK;
+}
+template <typename T>
+int launch_tline(const LineParams<T>& p, int ns, bool edge, cudaStream_t st) {
+    switch (ns) {
+        case 2: return launch_tline_ns<T, 2>(p, edge, st);
+        case 4: return launch_tline_ns<T, 4>(p, edge, st);
+        case 8: return launch_tline_ns<T, 8>(p, edge, st);
+        case 16: return launch_tline_ns<T, 16>(p, edge, st);
+        case 32:
+            if constexpr (sizeof(T) == 4) return launch_tline_ns<T, 32>(p, edge, st);
+    }
+    set_error("axis: no transposed line kernel for this extent");
+    return TS_EUNSUPPORTED;
+}
+
 // Where the lines of one launch lie: line l = group g = l / lines_inner, member m = l % lines_inner
 // starts at g * group_stride + m * line_stride; consecutive sites are site_stride apart.
 struct LineGeom {
@@ -1015,12 +1161,13 @@ struct LineGeom {
     int periodic;
     int64_t n_lines, line_stride, site_stride, lines_inner, group_stride;
     bool col;              // site_stride != 1: scalar accesses, adjacent lines in one block
+    bool transposed;       // strided lines of a state that does not stay in L2: one lane per line
 };
 LineGeom rows_of(const LatticeDesc& L) {
-    return LineGeom{L.nx, L.periodic_x, L.ny, L.nx, 1, L.ny, 0, false};
+    return LineGeom{L.nx, L.periodic_x, L.ny, L.nx, 1, L.ny, 0, false, false};
 }
 LineGeom cols_of(const LatticeDesc& L) {
-    return LineGeom{L.ny, L.periodic_y, L.nx, 1, L.nx, L.nx, 0, true};
+    return LineGeom{L.ny, L.periodic_y, L.nx, 1, L.nx, L.nx, 0, true, false};
 }
 
 // launch the line kernel on lines held completely in registers; p carries a chain (fill_chain) or
@@ -1037,6 +1184,13 @@ int launch_lines(const LineGeom& g, int dtype, LineParams<T>& p, T* re, T* im, c
     p.lines_inner = (int)g.lines_inner;
     p.group_stride = g.group_stride;
     p.periodic = g.periodic;
+    if (g.transposed) {
+        const TShape ts_ = tline_shape(g.n_sites, dtype);
+        if (ts_.ok()) {
+            p.n_warps = ts_.warps; p.n_lanes = 32; p.lines_per_block = 32;
+            return launch_tline<T>(p, ts_.ns, !g.periodic, st);
+        }
+    }
     const LineShape sh = line_shape(g.n_sites, dtype);
     if (!sh.ok()) { set_error("axis: line does not fit a thread block"); return TS_EUNSUPPORTED; }
     p.n_lanes = sh.lanes;
@@ -1437,9 +1591,9 @@ int axis_evolve(const LatticeDesc& L, void* psi_re, void* psi_im, void* scr_re, 
 namespace {
 LineGeom geom3(const Lattice3& L, int axis) {
     const int64_t plane = L.nx * L.ny;
-    if (axis == 0) return LineGeom{L.nx, L.per[0], L.ny * L.nz, L.nx, 1, L.ny * L.nz, 0, false};
-    if (axis == 1) return LineGeom{L.ny, L.per[1], L.nx * L.nz, 1, L.nx, L.nx, plane, true};
-    return LineGeom{L.nz, L.per[2], plane, 1, plane, plane, 0, true};
+    if (axis == 0) return LineGeom{L.nx, L.per[0], L.ny * L.nz, L.nx, 1, L.ny * L.nz, 0, false, false};
+    if (axis == 1) return LineGeom{L.ny, L.per[1], L.nx * L.nz, 1, L.nx, L.nx, plane, true, true};
+    return LineGeom{L.nz, L.per[2], plane, 1, plane, plane, 0, true, true};
 }
 const int kKindOfAxis[3] = {kKindLineRows, kKindLineCols, kKindLineZ};
 
