@@ -973,8 +973,10 @@ Angle odd_of(const StepCoef& c, bool col) {
 }
 
 // How a line of n sites is held: NS sites per lane, W warps.  One warp: any n = NS * lanes with
-// lanes <= 32; several warps: n = W * 32 * NS, W <= 16.  The smallest NS that fits (more lanes
-// and warps share the work of a line).
+// lanes <= 32 -- the smallest NS that fits (more lanes share the work of a line).  Several warps:
+// n = W * 32 * NS, W <= 16 -- the LARGEST NS that fits: the warps of a line meet at a barrier every
+// sub-step, so fewer warps with more in-lane work each is the cheaper cut (2048 sites: 2 warps of
+// 32 sites per lane, not 16 warps of 4).
 struct LineShape {
     int ns, warps, lanes;
     bool ok() const { return ns != 0; }
@@ -983,7 +985,13 @@ LineShape line_shape(int64_t n, int dtype) {
     const int ns_max = dtype == TS_F32 ? 32 : 16;
     for (int ns = 2; ns <= ns_max; ns *= 2)
         if (n % ns == 0 && n / ns <= 32) return {ns, 1, (int)(n / ns)};
-    for (int ns = 2; ns <= ns_max; ns *= 2)
+    static const bool small_ns = getenv("TS_PROBE_MW_SMALL") != nullptr;     // tuning probe only
+    if (small_ns) {
+        for (int ns = 2; ns <= ns_max; ns *= 2)
+            if (n % (32 * ns) == 0 && n / (32 * ns) <= kMaxLineWarps) return {ns, (int)(n / (32 * ns)), 32};
+        return {0, 0, 0};
+    }
+    for (int ns = ns_max; ns >= 2; ns /= 2)
         if (n % (32 * ns) == 0 && n / (32 * ns) <= kMaxLineWarps) return {ns, (int)(n / (32 * ns)), 32};
     return {0, 0, 0};
 }
@@ -1118,15 +1126,15 @@ int launch_line_t(const LineParams<T>& p, int ns, bool edge, bool col, cudaStrea
     return TS_EUNSUPPORTED;
 }
 
-// transposed strided lines: n = W * NS, W <= 16 warps; the largest W (most parallelism per line,
-// fewest registers per thread)
+// transposed strided lines: n = W * NS, W <= 16 warps; the largest NS (fewest warps at the barrier,
+// as for line_shape)
 struct TShape {
     int ns, warps;
     bool ok() const { return ns != 0; }
 };
 TShape tline_shape(int64_t n, int dtype) {
     const int ns_max = dtype == TS_F32 ? 32 : 16;
-    for (int ns = 2; ns <= ns_max; ns *= 2)
+    for (int ns = ns_max; ns >= 2; ns /= 2)
         if (n % ns == 0 && n / ns <= kTWarps) return {ns, (int)(n / ns)};
     return {0, 0};
 }
