@@ -317,6 +317,10 @@ def run_gpu(args):
         dist.init_process_group("nccl", device_id=dev)
 
     cfg = inputs.CONFIGS[args.config]
+    if args.scale:
+        # the config's recipe on an N x N lattice (not one of BASELINE.json's workloads: a size
+        # sweep of the same path; cpu_baseline then uses its bounded sample)
+        cfg = inputs.scaled(cfg, args.scale, args.scale)
     tdt = torch.float32 if cfg.dtype == "f32" else torch.float64
     eb = 4 if cfg.dtype == "f32" else 8
     re, im, _ = inputs.device_state(cfg, dev)
@@ -337,6 +341,8 @@ def run_gpu(args):
         plan.set_option("chain", args.chain)
     if args.variant:
         plan.set_option("variant", args.variant)
+    if args.ring_slots:
+        plan.set_option("ring_slots", args.ring_slots)
     c = cfg.coeffs()
     stream = torch.cuda.current_stream()
 
@@ -715,6 +721,9 @@ def main():
     ap.add_argument("--pot3d", action="store_true", help="with --lattice3d: a phase field")
     ap.add_argument("--chain", type=int, default=0, help="axis-split path: sub-steps per pass")
     ap.add_argument("--variant", type=int, default=0, help="plan option variant (0 = default path)")
+    ap.add_argument("--ring-slots", type=int, default=0, help="TMA ring: state row-pair slots per warp")
+    ap.add_argument("--scale", type=int, default=0,
+                    help="run the config's recipe on an N x N lattice instead (size sweeps)")
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: independent lattices per GPU (default, north_star) or one lattice "
                          "cut into row slabs with NCCL halo exchange")

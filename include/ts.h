@@ -105,8 +105,9 @@ int ts_evolve_3d(ts_plan* plan, void* psi_re, void* psi_im,
  *   cuda_stream      cudaStream_t passed as void* (NULL = legacy default stream).
  * Work is enqueued on the stream; the call does not synchronise.  The plan's scratch buffer is
  * in use until that work completes.
- * Errors: TS_EINVAL (NULL/misaligned/overlapping pointers, bad coefficients, n_steps < 0),
- * TS_EALLOC (scratch allocation), TS_ECUDA (launch failure; text in ts_last_error()).
+ * Errors: TS_EINVAL (NULL/misaligned/overlapping pointers, pointers to pageable host memory, bad
+ * coefficients, n_steps < 0), TS_EALLOC (scratch allocation), TS_ECUDA (launch failure; text in
+ * ts_last_error()).
  */
 int ts_evolve(ts_plan* plan, void* psi_re, void* psi_im,
               double a_half, double b_half, double a_full, double b_full,

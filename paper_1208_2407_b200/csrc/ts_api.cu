@@ -92,6 +92,17 @@ bool overlap(const void* a, const void* b, size_t bytes) {
     return x < y + bytes && y < x + bytes;
 }
 
+// a pointer the kernels can dereference: device or managed memory (or host memory registered with
+// CUDA); plain pageable host memory would fault inside the kernel
+bool device_accessible(const void* p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return false;
+    }
+    return a.type != cudaMemoryTypeUnregistered;
+}
+
 int ensure_alloc(void** p, size_t bytes) {
     if (*p) return TS_OK;
     cudaError_t e = cudaMalloc(p, bytes);
@@ -258,6 +269,8 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
     if (!aligned16(psi_re) || !aligned16(psi_im))
         return fail(TS_EINVAL, "device pointers must be 16-byte aligned");
     if (overlap(psi_re, psi_im, plane_bytes)) return fail(TS_EINVAL, "psi_re and psi_im overlap");
+    if (!device_accessible(psi_re) || !device_accessible(psi_im))
+        return fail(TS_EINVAL, "psi planes must be device memory (ts_evolve_host takes host planes)");
     bool any_pot = false, any_sep = false, can_v1 = true, can_stream = true;
     for (int k = 0; k < period; ++k) {
         const ts::StepCoef& c = pat[k].c;
@@ -268,6 +281,7 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
             const void* pot = ph.planes;
             any_pot = true;
             if (!aligned16(pot)) return fail(TS_EINVAL, "device pointers must be 16-byte aligned");
+            if (!device_accessible(pot)) return fail(TS_EINVAL, "pot_phase must be device memory");
             if (overlap(pot, psi_re, plane_bytes) || overlap(pot, psi_im, plane_bytes) ||
                 overlap((const char*)pot + plane_bytes, psi_re, plane_bytes) ||
                 overlap((const char*)pot + plane_bytes, psi_im, plane_bytes))
@@ -277,6 +291,8 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
             if (!ph.px || !ph.py) return fail(TS_EINVAL, "NULL separable phase vector");
             if (!aligned16(ph.px) || !aligned16(ph.py))
                 return fail(TS_EINVAL, "device pointers must be 16-byte aligned");
+            if (!device_accessible(ph.px) || !device_accessible(ph.py))
+                return fail(TS_EINVAL, "the separable phase vectors must be device memory");
         }
         can_v1 = can_v1 && ts::fused_supported(L, c);
         can_stream = can_stream && ts::stream_supported(L, c);
@@ -415,10 +431,10 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
     if (rc == TS_OK) rc = ensure_alloc(&plan->scratch_im, plane_bytes);
     if (rc != TS_OK) return rc;
 
-    // resident blocks per SM of the kernel that will run: the ring with phase planes is twice as
-    // large; fp64 pipelines beyond S = 2 take 255 registers
+    // resident blocks per SM of the kernel that will run: fp64 with phase planes (28 KB of rings per
+    // warp) or beyond S = 2 (255 registers) two, everything else three
     const bool planes = any_pot && !(any_sep && use_stream);
-    const int bpsm = (planes || (L.dtype == TS_F64 && S > 2)) ? 2 : 3;
+    const int bpsm = (L.dtype == TS_F64 && (planes || S > 2)) ? 2 : 3;
     const int seg = plan->opt_seg ? (int)plan->opt_seg : ts::fused_default_seg_rows(L, S, bpsm);
     plan->info_variant = use_stream ? 2 : 1;
     void* cur_re = psi_re; void* cur_im = psi_im;
@@ -486,6 +502,8 @@ int ts_evolve_3d(ts_plan* plan, void* psi_re, void* psi_im, double a_half, doubl
     if (!aligned16(psi_re) || !aligned16(psi_im) || (pot && !aligned16(pot)))
         return fail(TS_EINVAL, "device pointers must be 16-byte aligned");
     if (overlap(psi_re, psi_im, vol_bytes)) return fail(TS_EINVAL, "psi_re and psi_im overlap");
+    if (!device_accessible(psi_re) || !device_accessible(psi_im) || (pot && !device_accessible(pot)))
+        return fail(TS_EINVAL, "psi planes and pot_phase must be device memory");
     if (pot && (overlap(pot, psi_re, vol_bytes) || overlap(pot, psi_im, vol_bytes) ||
                 overlap((const char*)pot + vol_bytes, psi_re, vol_bytes) ||
                 overlap((const char*)pot + vol_bytes, psi_im, vol_bytes)))
@@ -551,8 +569,10 @@ int ts_slab_pass(ts_plan* plan, const void* src_re, const void* src_im, void* ds
     const size_t plane_bytes = (size_t)L.nx * (size_t)L.ny * plan->elem;
     const void* ptrs[10] = {src_re, src_im, dst_re, dst_im, up_re, up_im, dn_re, dn_im, phase_x,
                             phase_y};
-    for (const void* q : ptrs)
+    for (const void* q : ptrs) {
         if (q && !aligned16(q)) return fail(TS_EINVAL, "device pointers must be 16-byte aligned");
+        if (q && !device_accessible(q)) return fail(TS_EINVAL, "planes must be device (or peer-mapped) memory");
+    }
     if (overlap(src_re, dst_re, plane_bytes) || overlap(src_im, dst_im, plane_bytes) ||
         overlap(src_re, dst_im, plane_bytes) || overlap(src_im, dst_re, plane_bytes))
         return fail(TS_EINVAL, "ts_slab_pass works out of place: src and dst overlap");
@@ -686,6 +706,8 @@ int ts_plan_get_launch_times(ts_plan* plan, int max_n, int* kinds_out, float* ms
 int ts_norm(ts_plan* plan, const void* psi_re, const void* psi_im, double* out, void* cuda_stream) {
     if (!plan) return fail(TS_EINVAL, "NULL plan");
     if (!psi_re || !psi_im || !out) return fail(TS_EINVAL, "NULL argument");
+    if (!device_accessible(psi_re) || !device_accessible(psi_im))
+        return fail(TS_EINVAL, "psi planes must be device memory");
     int rc = check_device(plan);
     if (rc != TS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);

@@ -7,8 +7,9 @@
 // is therefore hidden by shared memory, not by registers, which removes the long-scoreboard
 // stalls that bound v1 (profiles/r1a_*): registers only hold the S+1 row pairs of the pipeline.
 // The register pipeline is unrolled over its rotation period S+1 so that rows never move between
-// registers.  Potential-phase rows travel in the same slots and are kept S+1 iterations longer,
-// because stage j of the pipeline applies the phase to rows that arrived j iterations earlier.
+// registers.  Potential-phase rows travel with the row pair (same copies batch, same mbarrier)
+// but land in a ring of their own, where they are kept S+1 iterations longer, because stage j of
+// the pipeline applies the phase to rows that arrived j iterations earlier.
 //
 // Results are written straight from registers with 128-bit stores into the other buffer
 // (double buffering); halo columns of a strip are recomputed and discarded
@@ -57,7 +58,8 @@ struct StreamParams {
     int py_off, py_n, py_wrap;   // separable phase: global row of local row 0, global height, wrap
     int nx, ny;
     int n_strips, wi, halo, seg_rows;
-    int nst;        // ring slots per warp
+    int nst;        // ring slots per warp (state row pairs)
+    int nph;        // with phase planes: slots of the separate phase ring (>= prefetch + S + 1)
     // tangents of the sweeps of the S chained sub-steps of this pass (angles may differ from
     // sub-step to sub-step: Eq. 4 chains U2 with three different time fractions)
     T te[TS_MAX_FUSE + 1];   // even sweeps: te[0] opening half sweep, te[j] the merged sweep between
@@ -77,6 +79,7 @@ struct StreamCtx {
     XCut e;              // where the lane's cross-lane X-odd pairs meet a closed edge
     T pxr[4], pxi[4];    // separable potential: phase factor of the lane's four columns
     uint32_t ring;       // shared address of the warp's slot ring
+    uint32_t pot_ring;   // ... of its phase ring (phase planes only)
     uint32_t lane_off;   // byte offset of the lane's 4 sites inside a row chunk
 };
 
@@ -196,8 +199,9 @@ struct Stages {
         if (PM == 1) {
             int s0 = cs - J;      if (s0 < 0) s0 += nst;
             int s1 = s0 - 1;      if (s1 < 0) s1 += nst;
-            const uint32_t pot_yj = c.ring + s0 * slotb + 4 * ROWB;
-            const uint32_t pot_yjm1 = c.ring + s1 * slotb + 6 * ROWB;
+            // cs / nst / slotb here: the PHASE ring's slot of this iteration, its length, 4 rows
+            const uint32_t pot_yj = c.pot_ring + s0 * slotb;
+            const uint32_t pot_yjm1 = c.pot_ring + s1 * slotb + 2 * ROWB;
             stream_stage<T, 1, BND, XEDGE, S, J>(p, c, y - 2 * J, a0, a1, g, h, pot_yj, pot_yjm1);
         } else if (PM == 2) {
             stream_stage<T, 2, BND, XEDGE, S, J>(p, c, y - 2 * J, a0, a1, g, h, 0, 0);
@@ -220,17 +224,23 @@ stream_kernel(const StreamParams<T> p) {
     // compiled in only there: as run-time branches it cost the closed kernels 13-18 %.
     constexpr bool PERX = BND == 1 || BND == 2 || BND == 4, PERY = BND == 1, SLAB = BND >= 3;
     const bool edge_top = !SLAB || p.edge_top, edge_bot = !SLAB || p.edge_bot;
-    constexpr bool POT = PM == 1;             // phase planes travel through the ring
-    constexpr int R = POT ? S + 1 : 1;        // iterations a ring slot stays live after its arrival
+    // Phase planes travel through a ring of their OWN (r2): a state row pair is consumed in the
+    // iteration it arrives, its phase rows are needed for S + 1 iterations (stage j applies P to
+    // rows that arrived j iterations ago).  In one ring every slot was 8 rows and lived S + 1
+    // iterations: 112 KB per block in fp32 at S = 3 (2 blocks per SM), 224 KB in fp64 (1 block).
+    // Split, the state ring is prefetch + 1 slots of 4 rows and the phase ring prefetch + S + 1.
+    constexpr bool POT = PM == 1;
+    constexpr int R = 1;                      // iterations a state slot stays live after its arrival
     constexpr uint32_t ROWB = kStripSites * sizeof(T);
-    constexpr int NROW = POT ? 8 : 4;         // re0 im0 re1 im1 [pr0 pi0 pr1 pi1]
-    constexpr uint32_t SLOTB = NROW * ROWB;
+    constexpr int NROW = POT ? 8 : 4;         // copies per iteration: re0 im0 re1 im1 [pr0 pi0 pr1 pi1]
+    constexpr uint32_t SLOTB = 4 * ROWB;      // a slot of either ring: four rows
 
     const int lane = threadIdx.x & 31;
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);   // warp-uniform
     const int strip = blockIdx.x * kWarps + warp;
     if (strip >= p.n_strips) return;
     const int NST = p.nst;
+    const int NPH = POT ? p.nph : 0;
     const int DIST = NST - R;                 // prefetch distance in iterations
 
     const int x0 = strip * p.wi;
@@ -241,9 +251,10 @@ stream_kernel(const StreamParams<T> p) {
     c.xedge = !PERX && (xs < 0 || xs + kStripSites > p.nx);
     c.e.up = !PERX && (xb == 0 || xb == p.nx);
     c.e.dn = !PERX && (xb + 4 == p.nx || xb + 4 == 0);
-    c.ring = smem_u32(smem_raw) + warp * NST * SLOTB;
+    c.ring = smem_u32(smem_raw) + warp * (NST + NPH) * SLOTB;
+    c.pot_ring = c.ring + NST * SLOTB;
     c.lane_off = lane * 4 * sizeof(T);
-    const uint32_t bars = smem_u32(smem_raw) + kWarps * NST * SLOTB + warp * NST * 8;
+    const uint32_t bars = smem_u32(smem_raw) + kWarps * (NST + NPH) * SLOTB + warp * NST * 8;
     const bool store_ok = (4 * lane >= p.halo) && (4 * lane < kStripSites - p.halo) && (xb < p.nx);
 
     // the strip window [xs, xs+128) as at most two contiguous global pieces (warp-uniform);
@@ -303,6 +314,7 @@ stream_kernel(const StreamParams<T> p) {
     int64_t foff = (int64_t)fy * p.nx;
     const int64_t plane_elems = (int64_t)p.nx * p.ny;
 
+    int fps = 0;                // phase-ring slot of the next fetch
     // fetch the next row pair into ring slot `slot` (one elected lane issues all copies)
     auto issue = [&](int slot) {
         // where the row pair lives: own planes -- or, beyond the slab, a neighbour's (ts_slab_pass)
@@ -328,11 +340,13 @@ stream_kernel(const StreamParams<T> p) {
                 const uint32_t dst = c.ring + slot * SLOTB;
                 const T* planes[8] = {b_re, b_im, b_re, b_im,
                                       p.pot_re, p.pot_im, p.pot_re, p.pot_im};
+                const uint32_t dst_p = c.pot_ring + fps * SLOTB;
 #pragma unroll
                 for (int r = 0; r < NROW; ++r) {
                     const T* row = planes[r] + (r < 4 ? off : foff) + ((r >> 1) & 1) * p.nx;
-                    bulk_g2s(dst + r * ROWB + dst_a, row + gx_a, bytes_a, bar);
-                    if (bytes_b) bulk_g2s(dst + r * ROWB + dst_b, row, bytes_b, bar);
+                    const uint32_t d = (r < 4 ? dst + r * ROWB : dst_p + (r - 4) * ROWB);
+                    bulk_g2s(d + dst_a, row + gx_a, bytes_a, bar);
+                    if (bytes_b) bulk_g2s(d + dst_b, row, bytes_b, bar);
                 }
             } else {
                 mbar_arrive(bar);
@@ -341,12 +355,14 @@ stream_kernel(const StreamParams<T> p) {
         fy += 2;
         foff += 2 * (int64_t)p.nx;
         if (PERY && fy >= p.ny) { fy -= p.ny; foff -= plane_elems; }
+        if (POT && ++fps == NPH) fps = 0;
     };
 
     for (int k = 0; k < DIST; ++k)
         if (k < n_iter) issue(k);
 
     int cs = 0;                 // ring slot of the current iteration
+    int ps = 0;                 // phase-ring slot of the current iteration
     uint32_t cph = 0;           // its mbarrier phase parity
     int rs = DIST % NST;        // ring slot refilled at the top of the current iteration
 
@@ -393,7 +409,8 @@ stream_kernel(const StreamParams<T> p) {
                     zero_row(x0);
                     zero_row(x1);
                 }
-                Stages<T, PM, BND, XEDGE, S, 0>::run(p, c, y, cs, NST, SLOTB, W, U, x0, x1);
+                if (POT) Stages<T, PM, BND, XEDGE, S, 0>::run(p, c, y, ps, NPH, SLOTB, W, U, x0, x1);
+                else Stages<T, PM, BND, XEDGE, S, 0>::run(p, c, y, cs, NST, SLOTB, W, U, x0, x1);
                 if (it >= 2 * S && store_ok && y - 2 * S < y_out1) {
                     const int64_t off = (int64_t)(y - 2 * S) * p.nx + xb;
                     st4(p.dst_re + off, x0.re, p.out_scale);
@@ -403,6 +420,7 @@ stream_kernel(const StreamParams<T> p) {
                 }
                 if (++cs == NST) { cs = 0; cph ^= 1; }
                 if (++rs == NST) rs = 0;
+                if (POT && ++ps == NPH) ps = 0;
             }
         };
         half(std::integral_constant<int, 0>{});
@@ -426,8 +444,8 @@ bool stream_pdl() {
 
 template <typename T, int S, int PM, int BND>
 int launch(const StreamParams<T>& p, cudaStream_t st) {
-    constexpr uint32_t SLOTB = (PM == 1 ? 8 : 4) * kStripSites * sizeof(T);
-    const size_t smem = (size_t)kWarps * p.nst * (SLOTB + 8);
+    constexpr uint32_t SLOTB = 4 * kStripSites * sizeof(T);
+    const size_t smem = (size_t)kWarps * ((size_t)(p.nst + (PM == 1 ? p.nph : 0)) * SLOTB + p.nst * 8);
     // register budget: the ring (64 KB per block) admits 3 blocks per SM anyway, so fp32 gets 168
     // registers from S = 3 on (128 below); fp64 3 or 2 blocks (255)
     constexpr int MINB = sizeof(T) == 4 ? (S <= 2 ? 4 : 3) : (S <= 2 ? 3 : 2);
@@ -519,12 +537,16 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
     p.wi = kStripSites - 2 * p.halo;
     p.n_strips = (int)((L.nx + p.wi - 1) / p.wi);
     p.seg_rows = seg_rows;
-    const int live = pot ? S + 1 : 1;
+    // state ring: prefetch distance + 1 slots; phase ring (planes only): prefetch + S + 1
     if (nst <= 0) nst = stream_default_slots(L, S, pot != nullptr);   // separable: as without
-    if (nst < live + 1) nst = live + 1;
-    const size_t slotb = (size_t)(pot ? 8 : 4) * kStripSites * sizeof(T);
-    while (nst > live + 1 && (size_t)kWarps * nst * (slotb + 8) > 227u * 1024u) --nst;
+    if (nst < 2) nst = 2;
+    const size_t slotb = (size_t)4 * kStripSites * sizeof(T);
+    auto smem_of = [&](int n) {
+        return (size_t)kWarps * ((size_t)(n + (pot ? n - 1 + S + 1 : 0)) * slotb + n * 8);
+    };
+    while (nst > 2 && smem_of(nst) > 227u * 1024u) --nst;
     p.nst = nst;
+    p.nph = pot ? nst - 1 + S + 1 : 0;
     // tangents and deferred cosines of the S sub-steps (all in double, rounded once).  The merged
     // even sweep between sub-steps j-1 and j rotates by the sum of their half angles:
     // cos = a a' - b b', sin = a b' + b a'.
@@ -637,9 +659,13 @@ int stream_default_steps_sep(const LatticeDesc& L) {
 
 int stream_default_slots(const LatticeDesc& L, int S, bool pot) {
     // measured on B200 (profiles/r1b_probe.txt): 8 row-pair slots per warp keep ~7 iterations in
-    // flight for fp32 without a potential (64 KB per block, 3 blocks per SM); with a potential a
-    // slot also carries the phase rows and stays live S+1 iterations, so S+4 leaves 3 in flight.
-    if (pot) return S + 4;
+    // flight for fp32 without a potential (64 KB per block, 3 blocks per SM).  With phase planes
+    // (own ring of prefetch + S + 1 slots) two state slots = one iteration in flight per warp, in
+    // both types: fp32 at S = 3 14 KB per warp, 3 blocks per SM (register-limited); fp64 28 KB per
+    // warp, 112 KB per block, 2 blocks per SM.  Measured (profiles/r2_probe_stream_pot.txt): C3
+    // 5.34e11 with one ring of 8-row slots, 5.76e11 with 3 state slots, 5.96e11 with 2; C5 2.81e11
+    // -> 3.05e11 with 2 (2.86e11 with 3: one block per SM again).
+    if (pot) return 2;
     return L.dtype == TS_F32 ? 8 : 6;
 }
 

@@ -195,3 +195,24 @@ def test_periodic_eigenstates_fused(sx, sy):
     got_re, got_im, info = G.gpu_evolve(cfg, psi0, np.zeros_like(psi0), None, n_steps=n, path=2)
     ph = np.exp(1j * 2 * n * theta * ((1 - 2 * sx) + (1 - 2 * sy)))
     assert np.abs((got_re + 1j * got_im) - ph * psi0).max() < 1e-15 * 50
+
+
+def test_pageable_host_pointers_are_rejected_not_dereferenced():
+    # include/ts.h: the planes are DEVICE memory; a pageable host pointer must come back as
+    # TS_EINVAL before anything is enqueued (it would fault inside the kernel)
+    import ctypes
+    import torch
+    from paper_1208_2407_b200 import binding
+    plan = binding.Plan(64, 64, torch.float32, "closed")
+    host = np.zeros((2, 64, 64), dtype=np.float32)
+    dev = torch.zeros((64, 64), device="cuda:0")
+    L = binding.lib()
+    hp = ctypes.c_void_p(host.ctypes.data)
+    rc = L.ts_evolve(plan._h, hp, ctypes.c_void_p(host[1].ctypes.data), 1.0, 0.0, 1.0, 0.0, None, 1, None)
+    assert rc == binding.TS_EINVAL and "device memory" in binding.last_error()
+    rc = L.ts_evolve(plan._h, ctypes.c_void_p(dev.data_ptr()), hp, 1.0, 0.0, 1.0, 0.0, None, 1, None)
+    assert rc == binding.TS_EINVAL
+    out = ctypes.c_double(0.0)
+    assert L.ts_norm(plan._h, hp, hp, ctypes.byref(out), None) == binding.TS_EINVAL
+    assert plan.info("launches") == 0
+    plan.destroy()
