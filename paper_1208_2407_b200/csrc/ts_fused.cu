@@ -261,7 +261,7 @@ int fused_default_seg_rows(const LatticeDesc& L, int S, int blocks_per_sm) {
     // One warp per (strip, segment), 4 strips per block; a segment recomputes 2S warm-up row pairs,
     // so its cost is seg/2 + 2S iterations: longer segments win until the grid no longer fills the
     // machine.  Pick the number of waves the cap on the segment height allows (256 rows, 512 for
-    // S >= 5: probes r1d), then the segment count that fills those waves and no more -- a grid of
+    // S >= 5: round-1 probes), then the segment count that fills those waves and no more -- a grid of
     // 1.1 waves costs two (4096^2: 490 blocks on 444 slots ran at 60 % of the 16384^2 rate).
     const int halo = (2 * S + 3) / 4 * 4;
     const int64_t strips = (L.nx + (kStripSites - 2 * halo) - 1) / (kStripSites - 2 * halo);
@@ -282,7 +282,7 @@ int fused_default_seg_rows(const LatticeDesc& L, int S, int blocks_per_sm) {
 }
 
 int fused_default_steps(const LatticeDesc& L, bool pot) {
-    // steps fused per pass, measured on B200 (profiles/r1d_probe.txt): fp32 without potential 6
+    // steps fused per pass, measured on B200 (round-1 probes): fp32 without potential 6
     // (regrouped sweeps, packed FMAs; ts_evolve clamps to what the chosen kernel has) -- 4 on
     // small lattices (below 8 M sites), where segments are short and the 2S warm-up iterations dominate; fp32 with
     // potential 3; fp64 3 with, 4 without.

@@ -60,7 +60,7 @@ __device__ __forceinline__ void rot(T& rp, T& ip, T& rq, T& iq, T t) {
 
 // Packed fp32 arithmetic (sm_100: fma.rn.f32x2 / mul.rn.f32x2, SASS FFMA2 / FMUL2): two FMAs per
 // issue slot on an aligned register pair.  The kernel is issue-limited before it is FMA-pipe
-// limited (profiles/r1b_*), so the sweeps whose pairs line up with adjacent sites use it.  ptxas
+// limited (round-1 captures), so the sweeps whose pairs line up with adjacent sites use it.  ptxas
 // folds the scalar broadcast, the negation and a swapped source pair into operand modifiers.
 // (dx, dy) = s * (bx, by) + (cx, cy)
 __device__ __forceinline__ void fma2(float& dx, float& dy, float s, float bx, float by, float cx,

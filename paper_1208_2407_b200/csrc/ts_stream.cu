@@ -5,7 +5,7 @@
 // rows are brought on chip by cp.async.bulk (TMA, completion on an mbarrier) into a ring of NST
 // row-pair slots owned by the warp, several iterations ahead of their use.  Global-load latency
 // is therefore hidden by shared memory, not by registers, which removes the long-scoreboard
-// stalls that bound v1 (profiles/r1a_*): registers only hold the S+1 row pairs of the pipeline.
+// stalls that bound v1 (round 1): registers only hold the S+1 row pairs of the pipeline.
 // The register pipeline is unrolled over its rotation period S+1 so that rows never move between
 // registers.  Potential-phase rows travel with the row pair (same copies batch, same mbarrier)
 // but land in a ring of their own, where they are kept S+1 iterations longer, because stage j of
@@ -373,7 +373,7 @@ stream_kernel(const StreamParams<T> p) {
     // into the first sweep of that stage), and a set is dead once its pair has left, so S+1 pairs
     // are live, exactly as in a rotation over S+1 sets -- but the loop repeats after TWO iterations
     // instead of S+1: the S+1-fold unrolled rotation of r1b was 41 KB of SASS at S = 4 and
-    // overflowed the instruction cache beyond (no_instruction stalls, profiles/r1d_*).
+    // overflowed the instruction cache beyond (no_instruction stalls, round-1 captures).
     // The whole loop exists twice for closed lattices: warps whose strip touches an edge in x or
     // whose segment touches one in y (the outer ring of the warp grid) carry per-lane couplings,
     // zero ghost sites and the 1/a factor of unpaired sites (XEDGE, branch-free selects); all
@@ -658,7 +658,7 @@ int stream_default_steps_sep(const LatticeDesc& L) {
 }
 
 int stream_default_slots(const LatticeDesc& L, int S, bool pot) {
-    // measured on B200 (profiles/r1b_probe.txt): 8 row-pair slots per warp keep ~7 iterations in
+    // measured on B200 (round-1 probes): 8 row-pair slots per warp keep ~7 iterations in
     // flight for fp32 without a potential (64 KB per block, 3 blocks per SM).  With phase planes
     // (own ring of prefetch + S + 1 slots) two state slots = one iteration in flight per warp, in
     // both types: fp32 at S = 3 14 KB per warp, 3 blocks per SM (register-limited); fp64 28 KB per
