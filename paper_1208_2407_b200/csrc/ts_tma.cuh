@@ -49,10 +49,26 @@ __device__ __forceinline__ void lds4(uint32_t addr, float (&v)[4]) {
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
                  : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]) : "r"(addr));
 }
+// fp64: a lane's four sites are 32 bytes, so two 16-byte loads at stride 32 over the lanes are
+// 2-way bank conflicts (39 % of the shared-memory wavefronts of the C5 kernel, ncu r2).  A 128-bit
+// load is served eight lanes at a time: lanes 0-3 of each eight read their first half first,
+// lanes 4-7 their second half -- 128 distinct bytes per eight lanes in both loads -- and the
+// halves are put back in order by selects.  addr is 32 * lane beyond a 128-byte aligned row.
+#ifndef TS_F64_PLAIN_LDS
+__device__ __forceinline__ void lds4(uint32_t addr, double (&v)[4]) {
+    const bool sw = (addr & 128u) != 0;
+    double a0, a1, b0, b1;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(a0), "=d"(a1) : "r"(addr + (sw ? 16u : 0u)));
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(b0), "=d"(b1) : "r"(addr + (sw ? 0u : 16u)));
+    v[0] = sw ? b0 : a0; v[1] = sw ? b1 : a1;
+    v[2] = sw ? a0 : b0; v[3] = sw ? a1 : b1;
+}
+#else
 __device__ __forceinline__ void lds4(uint32_t addr, double (&v)[4]) {
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[0]), "=d"(v[1]) : "r"(addr));
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v[2]), "=d"(v[3]) : "r"(addr + 16));
 }
+#endif
 
 // one lane per warp, known to the compiler as a single active lane (no per-lane issue loops)
 __device__ __forceinline__ bool elect_one() {
