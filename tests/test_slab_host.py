@@ -104,3 +104,20 @@ def test_pass_cutting_and_u4_pattern():
     flat = [c for p in passes for c in p]
     assert flat == pat * 4
     assert list(slab._passes([(1.0, 0.0, 1.0, 0.0)], 0, 6)) == []
+
+
+def test_u4_table_of_the_library_matches_eq4():
+    # ts_u4_coefficients (host arithmetic inside libts, no device needed) against the fractions of
+    # Eq. 4 as the oracle states them
+    import oracle
+    from paper_1208_2407_b200 import binding
+    theta = 0.37
+    rows = binding.u4_coefficients(theta)
+    assert len(rows) == 5
+    for row, f in zip(rows, oracle.u4_fractions()):
+        th = f * theta
+        want = (math.cos(th / 2), math.sin(th / 2), math.cos(th), math.sin(th))
+        assert max(abs(a - b) for a, b in zip(row, want)) < 1e-15
+    assert abs(sum(oracle.u4_fractions()) - 1.0) < 1e-15
+    with pytest.raises(binding.TsError):
+        binding.u4_coefficients(float("nan"))
