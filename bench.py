@@ -704,7 +704,11 @@ def run_gpu_slab(args):
                                    + ((" over NVLink peer memory" if fused_halo else " over NCCL")
                                       if world > 1 else " (one GPU, slabs stepped in turn)")),
                    "fuse_steps": S, "norm2_before": n0, "norm_drift": n1 / n0 - 1,
-                   "l2": "state far larger than the 126 MB L2; no flush"},
+                   "l2": "state far larger than the 126 MB L2; no flush",
+                   "note": ("N > 1 had NOT RUN on hardware when this was written (rounds 1-2 had "
+                            "one-GPU boxes only): NCCL halo exchange / symmetric-memory peer halos "
+                            "are covered by gloo and one-device tests, DESIGN.md 8") if world > 1
+                   else "one GPU: all slabs stepped in turn"},
         "clocks": clocks, "gpu_launches": launches * args.steps,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": None,
