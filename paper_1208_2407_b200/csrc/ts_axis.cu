@@ -731,6 +731,7 @@ struct YcolParams {
     T* dst_im;
     int nx, ny;
     int n_strips, seg_rows, nst;
+    int edge_rows;               // closed in y: rows of the short first and last segment (0: none)
     int periodic_y;
     Coef<T> te[kMaxChain + 1];   // even sweeps: opening half, S-1 merged, closing half
     Coef<T> to[kMaxChain];       // odd sweep of sub-step j (the caller's full-angle coefficients)
@@ -848,8 +849,23 @@ ycol_kernel(const __grid_constant__ YcolParams<T> p) {
     const uint32_t bars = smem_u32(smem_raw) + kYWarps * NST * SLOTB + warp * NST * 8;
     const uint32_t lane_off = lane * sizeof(T);
 
-    const int y_out0 = blockIdx.y * p.seg_rows;
-    const int y_out1 = min(y_out0 + p.seg_rows, p.ny);
+    // Closed lattices: the segments that touch row 0 / ny run the edge variant of the loop, which
+    // costs about 1.5x per row; as whole segments they ended every pass late (a closed 16384^2
+    // lattice was 21 % slower than a periodic one).  They are cut SHORT instead (edge_rows), so
+    // that the edge arithmetic covers a few per cent of the rows and those blocks finish early.
+    int y_out0, y_out1;
+    if (p.edge_rows > 0) {
+        const int last = (int)gridDim.y - 1;
+        if ((int)blockIdx.y == 0) { y_out0 = 0; y_out1 = p.edge_rows; }
+        else if ((int)blockIdx.y == last) { y_out0 = p.ny - p.edge_rows; y_out1 = p.ny; }
+        else {
+            y_out0 = p.edge_rows + ((int)blockIdx.y - 1) * p.seg_rows;
+            y_out1 = min(y_out0 + p.seg_rows, p.ny - p.edge_rows);
+        }
+    } else {
+        y_out0 = blockIdx.y * p.seg_rows;
+        y_out1 = min(y_out0 + p.seg_rows, p.ny);
+    }
     const int y_in0 = y_out0 - 2 * S;
     const int n_iter = ((y_out1 - y_out0) / 2 + 2 * S + 1) & ~1;
 
@@ -1312,7 +1328,9 @@ int launch_ycol(const YcolParams<T>& p, cudaStream_t st) {
         TS_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         if (dev >= 0 && dev < 64) configured[dev].store(smem, std::memory_order_relaxed);
     }
-    const int n_seg = (p.ny + p.seg_rows - 1) / p.seg_rows;
+    const int n_seg = p.edge_rows > 0
+                          ? 2 + (p.ny - 2 * p.edge_rows + p.seg_rows - 1) / p.seg_rows
+                          : (p.ny + p.seg_rows - 1) / p.seg_rows;
     dim3 grid((p.n_strips + kYWarps - 1) / kYWarps, n_seg);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid;
@@ -1348,6 +1366,14 @@ int ycol_depth(int n, int dtype) {
 }
 int ycol_blocks_per_sm(int S, int dtype, bool uni) { return ycol_blocks_for(S, dtype == TS_F32 ? 1 : 2, uni); }
 
+// rows of the short first / last segment of a lattice that is closed in y (0: uniform segments):
+// where the interior is worth several segments
+constexpr int kEdgeRows = 128;
+int ycol_edge_rows(const LatticeDesc& L, int seg_rows) {
+    return (!L.periodic_y && L.ny >= 2 * kEdgeRows + 4 * (int64_t)seg_rows && seg_rows > kEdgeRows)
+               ? kEdgeRows : 0;
+}
+
 // One pipelined pass along the columns: sub-steps subs[0 .. n) chained, padded with identity
 // sub-steps (zero angle) up to the instantiated depth S.
 template <typename T>
@@ -1360,6 +1386,7 @@ int ycol_pass(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re,
     p.seg_rows = seg_rows;
     p.nst = nst;
     p.periodic_y = L.periodic_y;
+    p.edge_rows = ycol_edge_rows(L, seg_rows);
     double log_scale = 0.0;
     Angle prev{1.0, 0.0};
     for (int j = 0; j <= kMaxChain; ++j) p.te[j] = Coef<T>{T(0), T(0)};
@@ -1413,9 +1440,16 @@ int ycol_default_seg(const LatticeDesc& L, int S, bool uni) {
         r += r % 2;
         if (r < 16 && segs > 1) break;
         if (r > cap) continue;
-        const int64_t n_seg = (L.ny + r - 1) / r;
-        const int64_t waves = (n_seg * blocks_x + slots - 1) / slots;
-        const int64_t cost = waves * (r + 4 * S);
+        // closed lattices: two short edge segments besides the interior ones; a block of theirs is
+        // the fraction 1.5 (e + 4S) / (r + 4S) of an interior block (the edge variant of the loop
+        // costs about half as much again per row).  Without them the first and last segment run
+        // the edge variant as a whole.
+        const int64_t e = ycol_edge_rows(L, (int)r);
+        const int64_t n_seg = e ? 2 + (L.ny - 2 * e + r - 1) / r : (L.ny + r - 1) / r;
+        double eff = (double)n_seg * blocks_x;
+        if (e) eff += 2.0 * blocks_x * (1.5 * (e + 4 * S) / (double)(r + 4 * S) - 1.0);
+        const int64_t waves = (int64_t)ceil(eff / (double)slots - 1e-9);
+        const int64_t cost = waves * (r + 4 * S) * ((!L.periodic_y && e == 0) ? 3 : 2);
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_seg = r; }
         if (n_seg * blocks_x > 64 * slots) break;
     }

@@ -169,3 +169,15 @@ def test_periodic_eigenstates(sx, sy):
     got_re, got_im, info = G.gpu_evolve(cfg, psi0, np.zeros_like(psi0), None, n_steps=n, variant=4)
     ph = np.exp(1j * 2 * n * theta * ((1 - 2 * sx) + (1 - 2 * sy)))
     assert np.abs((got_re + 1j * got_im) - ph * psi0).max() < 1e-15 * 200
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("boundary", ["closed", "periodic"])
+@pytest.mark.parametrize("seg_rows,chain", [(260, 8), (300, 12), (514, 4)])
+def test_short_edge_segments_of_the_column_pipeline(dtype, boundary, seg_rows, chain):
+    # closed lattices: the first and last 128 rows are segments of their own (they run the edge
+    # variant of the loop), the interior is cut into seg_rows; 2050 rows fit no lane layout, so the
+    # columns are pipelined
+    cfg = G.make_cfg(128, 2050, dtype, boundary, 0.3, 13)
+    info = check(cfg, 13, 5 * seg_rows + chain, chain=chain, seg_rows=seg_rows)
+    assert info["seg_rows"] == seg_rows and info["chain_y"] <= chain
