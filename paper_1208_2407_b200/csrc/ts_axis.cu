@@ -29,6 +29,14 @@
 //                 columns, one per lane, S <= 24 chained sub-steps in flight, rows brought in by
 //                 bulk async copies (TMA) into a per-warp shared-memory ring.  No x halo at all;
 //                 4S warm-up rows per segment.
+//   tline_kernel  strided lines of a state that does not stay in L2 (y and z of a 3-D lattice):
+//                 one LANE per line, 32 adjacent lines per warp (coalesced rows), the line cut
+//                 over the warps of the block.
+//
+// The resident kernels use the IN-PLACE form of the rotation (first += i k1 second, then
+// second += i k2 first') with one scale per index parity followed on the host -- see SubCoef --
+// and can run, instead of a chain, a short sweep PROGRAM followed by the potential phase (the
+// per-axis regrouping of 3-D steps with a potential, axis3_evolve).
 //
 // A site is held as the register pair (re, im), so that EVERY pair rotation, even or odd, is two
 // packed FMAs:  (p.re, p.im) += (-t, t) * (q.im, q.re)  and the same with p and q exchanged
