@@ -41,6 +41,7 @@
 // A site is held as the register pair (re, im), so that EVERY pair rotation, even or odd, is two
 // packed FMAs:  (p.re, p.im) += (-t, t) * (q.im, q.re)  and the same with p and q exchanged
 // (sm_100 fma.rn.f32x2; ptxas folds the swapped source pair into an operand modifier).
+#include <cuda.h>       // CUtensorMap and its enums only: the encoder is fetched from the runtime
 #include <math.h>
 #include <stdlib.h>
 #include <string.h>
@@ -52,6 +53,10 @@
 #include "ts_internal.h"
 #include "ts_rows.cuh"
 #include "ts_tma.cuh"
+
+#ifndef TS_YCOL_TMAP
+#define TS_YCOL_TMAP 1      // column pipeline: rows fetched by 2-D tensor-map copies (0: 1-D bulk copies)
+#endif
 
 namespace ts {
 namespace {
@@ -839,7 +844,11 @@ constexpr int ycol_min_blocks() {
 
 template <typename T, int S, bool PERY, bool UNI>
 __global__ void __launch_bounds__(kYWarps * 32, ycol_min_blocks<T, S, UNI>())
-ycol_kernel(const __grid_constant__ YcolParams<T> p) {
+ycol_kernel(const __grid_constant__ YcolParams<T> p
+#if TS_YCOL_TMAP
+            , const __grid_constant__ CUtensorMap tm_re, const __grid_constant__ CUtensorMap tm_im
+#endif
+) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr uint32_t ROWB = kYCols * sizeof(T);
     constexpr uint32_t SLOTB = 4 * ROWB;          // re0 im0 re1 im1
@@ -888,12 +897,36 @@ ycol_kernel(const __grid_constant__ YcolParams<T> p) {
 
     // running fetch position (warp-uniform): rows (fy, fy+1) of the strip's columns
     int fy = PERY ? rows::wrap_index(y_in0, p.ny) : y_in0;
+    uint32_t f_dst = ring, f_bar = bars;
+    int f_slot = 0;
+#if TS_YCOL_TMAP
+    // One tensor-map copy per plane and iteration: the box is 32 columns x 2 rows at element
+    // coordinates (x0c, fy) -- no 64-bit address arithmetic in the loop (the four 1-D bulk copies
+    // per iteration cost ~38 uniform-datapath instructions of 180, ncu r2), columns beyond the
+    // lattice arrive as zeros.  Slot layout: re row 0, re row 1, im row 0, im row 1.
+    (void)bytes;
+    auto issue = [&]() {
+        const bool rowok = PERY || (fy >= 0 && fy < p.ny);
+        if (leader) {
+            if (rowok) {
+                mbar_arrive_expect_tx(f_bar, 4 * ROWB);
+                tensor2d_g2s(f_dst, &tm_re, x0c, fy, f_bar);
+                tensor2d_g2s(f_dst + 2 * ROWB, &tm_im, x0c, fy, f_bar);
+            } else {
+                mbar_arrive(f_bar);
+            }
+        }
+        fy += 2;
+        if (PERY && fy >= p.ny) fy -= p.ny;
+        f_dst += SLOTB; f_bar += 8;
+        if (++f_slot == NST) { f_slot = 0; f_dst = ring; f_bar = bars; }
+    };
+    constexpr uint32_t kOffAim = 2 * ROWB, kOffBre = ROWB;      // a = row 0, b = row 1 of the pair
+#else
     const int64_t pitchB = (int64_t)p.nx * sizeof(T);
     const int64_t planeB = pitchB * p.ny;
     const char* f_re = reinterpret_cast<const char*>(p.src_re + x0c) + (int64_t)fy * pitchB;
     const char* f_im = reinterpret_cast<const char*>(p.src_im + x0c) + (int64_t)fy * pitchB;
-    uint32_t f_dst = ring, f_bar = bars;
-    int f_slot = 0;
     auto issue = [&]() {
         const bool rowok = PERY || (fy >= 0 && fy < p.ny);
         if (leader) {
@@ -912,6 +945,8 @@ ycol_kernel(const __grid_constant__ YcolParams<T> p) {
         f_dst += SLOTB; f_bar += 8;
         if (++f_slot == NST) { f_slot = 0; f_dst = ring; f_bar = bars; }
     };
+    constexpr uint32_t kOffAim = ROWB, kOffBre = 2 * ROWB;      // re0 im0 re1 im1
+#endif
     // the ring is filled completely; iteration i lives in slot i mod NST and is refilled, for
     // iteration i + NST, at the top of iteration i + 1 (when its values have been consumed)
     for (int k = 0; k < NST; ++k)
@@ -936,8 +971,8 @@ ycol_kernel(const __grid_constant__ YcolParams<T> p) {
         auto fetch_regs = [&](int y, Cx<T>& a, Cx<T>& b) {
             const bool rowok = !EDGE || (y >= 0 && y < p.ny);
             if (rowok) {
-                a.re = lds1(l_src, T()); a.im = lds1(l_src + ROWB, T());
-                b.re = lds1(l_src + 2 * ROWB, T()); b.im = lds1(l_src + 3 * ROWB, T());
+                a.re = lds1(l_src, T()); a.im = lds1(l_src + kOffAim, T());
+                b.re = lds1(l_src + kOffBre, T()); b.im = lds1(l_src + 3 * ROWB, T());
             } else {
                 a.re = a.im = b.re = b.im = T(0);
             }
@@ -1324,6 +1359,43 @@ int xwin_pass(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re,
     return TS_OK;
 }
 
+#if TS_YCOL_TMAP
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled() {
+    static EncodeTiledFn fn = [] {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess) {
+            (void)cudaGetLastError();
+            f = nullptr;
+        }
+        return (EncodeTiledFn)f;
+    }();
+    return fn;
+}
+// a plane [ny][nx] of T as a 2-D tensor, box = 32 columns x 2 rows
+template <typename T>
+int plane_map(CUtensorMap* m, const T* plane, int nx, int ny) {
+    EncodeTiledFn enc = encode_tiled();
+    if (!enc) { set_error("cuTensorMapEncodeTiled is not available from this driver"); return TS_ECUDA; }
+    const cuuint64_t dims[2] = {(cuuint64_t)nx, (cuuint64_t)ny};
+    const cuuint64_t strides[1] = {(cuuint64_t)nx * sizeof(T)};
+    const cuuint32_t box[2] = {(cuuint32_t)kYCols, 2};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = enc(m, sizeof(T) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64,
+                           2, const_cast<T*>(plane), dims, strides, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                           CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled failed"); return TS_ECUDA; }
+    return TS_OK;
+}
+#endif
+
 template <typename T, int S, bool PERY, bool UNI>
 int launch_ycol(const YcolParams<T>& p, cudaStream_t st) {
     constexpr uint32_t SLOTB = 4 * kYCols * sizeof(T);
@@ -1351,7 +1423,15 @@ int launch_ycol(const YcolParams<T>& p, cudaStream_t st) {
     cfg.attrs = attr;
     // as in ts_stream.cu: dependent launch only for grids of at most one wave
     cfg.numAttrs = ((int64_t)grid.x * grid.y <= (int64_t)sm_count() * ycol_min_blocks<T, S, UNI>()) ? 1 : 0;
+#if TS_YCOL_TMAP
+    alignas(64) CUtensorMap tm_re, tm_im;
+    int rc = plane_map<T>(&tm_re, p.src_re, p.nx, p.ny);
+    if (rc == TS_OK) rc = plane_map<T>(&tm_im, p.src_im, p.nx, p.ny);
+    if (rc != TS_OK) return rc;
+    TS_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, p, tm_re, tm_im));
+#else
     TS_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, p));
+#endif
     return TS_OK;
 }
 

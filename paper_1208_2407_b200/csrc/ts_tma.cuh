@@ -45,6 +45,18 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
         : "memory");
 }
 
+// global -> shared copy of one box of a 2-D tensor map (TMA, SASS UTMALDG): coordinates in
+// elements (c0 = fastest dimension); elements of the box outside the tensor arrive as zeros and
+// count towards the transaction bytes like any others
+__device__ __forceinline__ void tensor2d_g2s(uint32_t dst, const void* tmap, int c0, int c1,
+                                             uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes "
+        "[%0], [%1, {%2, %3}], [%4];"
+        ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(c0), "r"(c1), "r"(bar)
+        : "memory");
+}
+
 __device__ __forceinline__ void lds4(uint32_t addr, float (&v)[4]) {
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
                  : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]) : "r"(addr));
