@@ -214,6 +214,31 @@ int ts_norm(ts_plan* plan, const void* psi_re, const void* psi_im,
             double* out_norm2_host, void* cuda_stream);
 
 /*
+ * ts_norm_static -- the same squared norm for callers that cannot call cudaMalloc
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid it): needs no plan,
+ * allocates NOTHING (no cudaMalloc / cudaFree, no stream or event creation), never synchronises.
+ * The per-chunk partial sums live in a 256 KB array in the library's device image (every GPU that
+ * loads libts holds it until the process exits) instead of a plan-owned allocation.
+ *   dtype              TS_F32 / TS_F64, the element type of both planes.
+ *   psi_re, psi_im     DEVICE pointers to n_sites elements each (read only; any lattice shape,
+ *                      planes contiguous).
+ *   n_sites            0 <= n_sites <= 536870912 (2^29: 32768 partial sums of 16384 sites; C4's
+ *                      16384^2 is 2^28).  Larger: TS_EUNSUPPORTED, nothing enqueued -- use ts_norm.
+ *   out_norm2_device   DEVICE pointer to one double, written by the last kernel of the call
+ *                      (stream-ordered: read it after the stream has reached that point).
+ * Enqueues two kernels on cuda_stream (on the current device) and returns.  The sum is taken in a
+ * fixed order, so equal inputs give bit-equal results.  The first call on each device looks up
+ * the array's device address (make that call outside a graph capture).
+ * Sharing: all calls on one device use the same array, which keeps the last call's contents;
+ * nothing in it needs clearing (a call reads only what it has itself just written), but two
+ * calls that OVERLAP on the GPU (different streams without a dependency) race -- order them.
+ * Errors: TS_EINVAL (NULL / host pointers, bad dtype, n_sites < 0), TS_EUNSUPPORTED (n_sites
+ * beyond the maximum), TS_ECUDA.
+ */
+int ts_norm_static(int dtype, const void* psi_re, const void* psi_im, int64_t n_sites,
+                   double* out_norm2_device, void* cuda_stream);
+
+/*
  * ts_evolve_host -- the same operation for HOST-resident planes (pageable or pinned): copies
  * psi (and pot_phase when given) to plan-owned device buffers, runs ts_evolve, copies psi
  * back, and synchronises.  This is the end-to-end entry measured by bench.py's "e2e".

@@ -14,7 +14,7 @@ _LIB_PATH = Path(__file__).resolve().parent / "libts.so"
 _lib = None
 
 SYMBOLS = ["ts_plan_create", "ts_plan_create_xy", "ts_plan_create_3d", "ts_evolve", "ts_evolve_3d", "ts_evolve_u4", "ts_evolve_sep", "ts_evolve_tdep", "ts_slab_pass",
-           "ts_norm", "ts_evolve_host", "ts_plan_set_option",
+           "ts_norm", "ts_norm_static", "ts_evolve_host", "ts_plan_set_option",
            "ts_plan_get_info", "ts_u4_coefficients", "ts_plan_reserve", "ts_plan_get_launch_times", "ts_plan_destroy",
            "ts_last_error"]
 
@@ -61,6 +61,8 @@ def lib():
         L.ts_slab_pass.restype = i32
         L.ts_norm.argtypes = [vp, vp, vp, ctypes.POINTER(dbl), vp]
         L.ts_norm.restype = i32
+        L.ts_norm_static.argtypes = [i32, vp, vp, i64, vp, vp]
+        L.ts_norm_static.restype = i32
         L.ts_evolve_host.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, vp, i64]
         L.ts_evolve_host.restype = i32
         L.ts_plan_set_option.argtypes = [vp, ctypes.c_char_p, i64]
@@ -112,6 +114,24 @@ def _stream_handle(stream):
     if stream is None:
         stream = torch.cuda.current_stream()
     return ctypes.c_void_p(stream.cuda_stream)
+
+
+def norm_static(psi_re, psi_im, out, stream=None) -> None:
+    """ts_norm_static: sum |psi|^2 into the one-element float64 DEVICE tensor `out`, without any
+    allocation and without a synchronisation (the partial sums live in a fixed 256 KB array of
+    the library's device image; at most 2^29 sites; calls that overlap on the GPU race)."""
+    import torch
+    if not (psi_re.is_cuda and psi_im.is_cuda and out.is_cuda):
+        raise ValueError("psi planes and out must be CUDA tensors")
+    if psi_re.dtype != psi_im.dtype or psi_re.shape != psi_im.shape:
+        raise ValueError("psi_re and psi_im must have the same dtype and shape")
+    if not (psi_re.is_contiguous() and psi_im.is_contiguous()):
+        raise ValueError("psi planes must be contiguous")
+    if out.dtype != torch.float64 or out.numel() != 1:
+        raise ValueError("out must be one float64 element")
+    _check(lib().ts_norm_static(_dtype_code(psi_re.dtype), ctypes.c_void_p(psi_re.data_ptr()),
+                                ctypes.c_void_p(psi_im.data_ptr()), int(psi_re.numel()),
+                                ctypes.c_void_p(out.data_ptr()), _stream_handle(stream)))
 
 
 class Plan:

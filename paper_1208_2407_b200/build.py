@@ -15,10 +15,11 @@ INCLUDE = PKG.parent / "include"
 LIB = PKG / "libts.so"
 # (source, object stem, extra flags); ts_stream.cu is compiled once per dtype so that its kernel
 # instantiations build in parallel
-SOURCES = ["ts_api.cu", "ts_generic.cu", "ts_fused.cu", "ts_stream.cu", "ts_tiny.cu", "ts_axis.cu"]
+SOURCES = ["ts_api.cu", "ts_generic.cu", "ts_fused.cu", "ts_stream.cu", "ts_tiny.cu", "ts_axis.cu",
+           "ts_noalloc.cu"]
 UNITS = [("ts_api.cu", "ts_api", []), ("ts_generic.cu", "ts_generic", []),
          ("ts_fused.cu", "ts_fused", []), ("ts_tiny.cu", "ts_tiny", []),
-         ("ts_axis.cu", "ts_axis", []),
+         ("ts_axis.cu", "ts_axis", []), ("ts_noalloc.cu", "ts_noalloc", []),
          ("ts_stream.cu", "ts_stream_f32", ["-DTS_STREAM_TU=32"]),
          ("ts_stream.cu", "ts_stream_f64", ["-DTS_STREAM_TU=64"])]
 HEADERS = [CSRC / "ts_internal.h", CSRC / "ts_rows.cuh", CSRC / "ts_tma.cuh", INCLUDE / "ts.h"]
