@@ -435,7 +435,9 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
     // warp) or beyond S = 2 (255 registers) two, everything else three
     const bool planes = any_pot && !(any_sep && use_stream);
     const int bpsm = (L.dtype == TS_F64 && (planes || S > 2)) ? 2 : 3;
-    const int seg = plan->opt_seg ? (int)plan->opt_seg : ts::fused_default_seg_rows(L, S, bpsm);
+    const int seg = plan->opt_seg ? (int)plan->opt_seg
+                    : use_stream ? ts::stream_default_seg_rows(L, S, bpsm)
+                                 : ts::fused_default_seg_rows(L, S, bpsm);
     plan->info_variant = use_stream ? 2 : 1;
     void* cur_re = psi_re; void* cur_im = psi_im;
     void* nxt_re = plan->scratch_re; void* nxt_im = plan->scratch_im;
@@ -606,7 +608,7 @@ int ts_slab_pass(ts_plan* plan, const void* src_re, const void* src_im, void* ds
     if (rc != TS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
     const ts::Peers peers{up_re, up_im, up_rows, dn_re, dn_im, dn_rows};
-    const int seg = plan->opt_seg ? (int)plan->opt_seg : ts::fused_default_seg_rows(L, n_sub, 3);
+    const int seg = plan->opt_seg ? (int)plan->opt_seg : ts::stream_default_seg_rows(L, n_sub, 3);
     rc = ts::stream_pass(L, src_re, src_im, dst_re, dst_im, subs, ph, n_sub, seg,
                          (int)plan->opt_slots, st, &peers);
     if (rc != TS_OK) return rc;

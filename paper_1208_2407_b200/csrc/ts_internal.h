@@ -114,6 +114,7 @@ bool stream_supported(const LatticeDesc& L, const StepCoef& c);
 int stream_max_steps(const LatticeDesc& L, bool pot);   // 6 for fp32 without potential, else 4
 int stream_default_steps_sep(const LatticeDesc& L);     // sub-steps per pass, separable phase
 int stream_default_slots(const LatticeDesc& L, int S, bool pot);
+int stream_default_seg_rows(const LatticeDesc& L, int S, int blocks_per_sm = 3);
 // One pass: dst <- U2(subs[S-1]) ... U2(subs[0]) src; the S sub-steps may have different angles
 // (fourth-order step, Eq. 4) but share one potential-phase array.
 int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,

@@ -57,7 +57,7 @@ struct StreamParams {
     int edge_top, edge_bot;   // closed in y: row 0 / row ny-1 is a lattice edge (not a cut)
     int py_off, py_n, py_wrap;   // separable phase: global row of local row 0, global height, wrap
     int nx, ny;
-    int n_strips, wi, halo, seg_rows;
+    int n_strips, wi, halo, seg_rows, n_seg;
     int nst;        // ring slots per warp (state row pairs)
     int nph;        // with phase planes: slots of the separate phase ring (>= prefetch + S + 1)
     // tangents of the sweeps of the S chained sub-steps of this pass (angles may differ from
@@ -237,8 +237,15 @@ stream_kernel(const StreamParams<T> p) {
 
     const int lane = threadIdx.x & 31;
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);   // warp-uniform
-    const int strip = blockIdx.x * kWarps + warp;
-    if (strip >= p.n_strips) return;
+    // (strip, segment) pairs are numbered strip-fastest and dealt to warps in order, so a block
+    // may hold the last strips of one segment and the first of the next: no warp slot idles when
+    // n_strips is not a multiple of kWarps (4096^2 at S = 3: 37 strips, 48 segments = 1776 warps,
+    // exactly one wave of 444 blocks; with a grid of (10, 44) three warps in forty were empty and
+    // every warp had 8 more rows).  Warps share nothing (own ring, own barriers).
+    const int wid = blockIdx.x * kWarps + warp;
+    const int segi = wid / p.n_strips;
+    const int strip = wid - segi * p.n_strips;
+    if (segi >= p.n_seg) return;
     const int NST = p.nst;
     const int NPH = POT ? p.nph : 0;
     const int DIST = NST - R;                 // prefetch distance in iterations
@@ -275,7 +282,7 @@ stream_kernel(const StreamParams<T> p) {
     const uint32_t slot_tx = NROW * (bytes_a + bytes_b);
     const uint32_t dst_a = off_a * sizeof(T), dst_b = bytes_a;
 
-    const int y_out0 = blockIdx.y * p.seg_rows;
+    const int y_out0 = segi * p.seg_rows;
     const int y_out1 = min(y_out0 + p.seg_rows, p.ny);
     const int y_in0 = y_out0 - 2 * S;
     // even, so that the two-iteration loop body has no conditional half (the extra iteration only
@@ -461,13 +468,12 @@ int launch(const StreamParams<T>& p, cudaStream_t st) {
                                          (int)smem));
         if (dev >= 0 && dev < kMaxDevices) configured[dev].store(smem, std::memory_order_relaxed);
     }
-    const int n_seg = (p.ny + p.seg_rows - 1) / p.seg_rows;
-    dim3 grid((p.n_strips + kWarps - 1) / kWarps, n_seg);
+    dim3 grid((unsigned)(((int64_t)p.n_strips * p.n_seg + kWarps - 1) / kWarps));
     // programmatic dependent launch pays where launch latency and the prologue are a visible part
     // of a pass, i.e. for grids of at most one wave (1024^2 +12 %, 2048^2 +17 %, 4096^2 +0-2 %);
     // on many-wave grids the next pass's blocks then start in lockstep and a 16384^2 pass gets
     // ~8 % slower (probe r1f pdl/pdl2), so those keep the ordinary launch
-    if (stream_pdl() && (int64_t)grid.x * grid.y <= 148 * 3) {
+    if (stream_pdl() && (int64_t)grid.x <= 148 * 3) {
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = grid;
         cfg.blockDim = dim3(kWarps * 32);
@@ -537,6 +543,7 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
     p.wi = kStripSites - 2 * p.halo;
     p.n_strips = (int)((L.nx + p.wi - 1) / p.wi);
     p.seg_rows = seg_rows;
+    p.n_seg = (int)((L.ny + seg_rows - 1) / seg_rows);
     // state ring: prefetch distance + 1 slots; phase ring (planes only): prefetch + S + 1
     if (nst <= 0) nst = stream_default_slots(L, S, pot != nullptr);   // separable: as without
     if (nst < 2) nst = 2;
@@ -667,6 +674,28 @@ int stream_default_slots(const LatticeDesc& L, int S, bool pot) {
     // -> 3.05e11 with 2 (2.86e11 with 3: one block per SM again).
     if (pot) return 2;
     return L.dtype == TS_F32 ? 8 : 6;
+}
+
+int stream_default_seg_rows(const LatticeDesc& L, int S, int blocks_per_sm) {
+    // As fused_default_seg_rows (a segment costs seg/2 + 2S iterations; whole waves, since a grid
+    // of 1.1 waves costs two), but counted in WARPS: the kernel deals (strip, segment) pairs to
+    // warps without gaps, so the machine holds 148 * blocks_per_sm * kWarps of them per wave
+    // whatever n_strips is.
+    const int halo = (2 * S + 3) / 4 * 4;
+    const int64_t strips = (L.nx + (kStripSites - 2 * halo) - 1) / (kStripSites - 2 * halo);
+    const int64_t slots = 148 * (int64_t)(blocks_per_sm > 0 ? blocks_per_sm : 3) * kWarps;
+    const int64_t cap = S >= 5 ? 512 : 256;
+    const int64_t min_segs = (L.ny + cap - 1) / cap;
+    int64_t waves = (min_segs * strips + slots - 1) / slots;
+    if (waves < 1) waves = 1;
+    int64_t segs = waves * slots / strips;
+    if (segs < 1) segs = 1;
+    int64_t r = (L.ny + segs - 1) / segs;
+    r += r % 2;
+    if (r > cap) r = cap;
+    if (r < 8) r = 8;     // small lattices: parallelism over warm-up redundancy
+    if (r > L.ny) r = L.ny;
+    return (int)r;
 }
 
 int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
