@@ -301,8 +301,15 @@ __device__ __forceinline__ void run_chain(const LineParams<T>& p, Line<T, NS>& L
     line_even_all(L, p.open1, p.open2);
     if (p.n_tab == 1) {
         const SubCoef<T> c = p.tab[0];
+        // counted down in 32 bits: no loop bound to re-read, no 64-bit compare in the inner loop
+        int64_t left = p.n_sub - 1;
 #pragma unroll 1
-        for (int64_t s = 1; s < p.n_sub; ++s) substep(c, c.e1, c.e2);
+        while (left > 0) {
+            const int n = left > (1 << 30) ? (1 << 30) : (int)left;
+            left -= n;
+#pragma unroll 1
+            for (int s = n; s > 0; --s) substep(c, c.e1, c.e2);
+        }
         substep(c, p.close1, p.close2);
     } else {
         int j = 0;
@@ -405,7 +412,8 @@ __device__ __forceinline__ void ld_if(bool pred, uint32_t addr, Cx<double>& v) {
 // registers and shuffles; MW = true: n_warps warps per line, the pair that straddles two warps
 // exchanged through shared memory.  In place: a line is read completely before it is written.
 template <typename T, int NS, bool EDGE, bool COL, bool MW>
-__global__ void __launch_bounds__(MW ? 512 : 128, MW ? 1 : (sizeof(T) * NS >= 128 ? 3 : 4))
+__global__ void __launch_bounds__(MW ? (sizeof(T) * NS >= 256 ? 256 : 512) : 128,
+                                  MW ? 1 : (sizeof(T) * NS >= 128 ? 3 : 4))
 line_kernel(const __grid_constant__ LineParams<T> p) {
     constexpr int PW = (Piece<T>::n < NS) ? Piece<T>::n : NS;     // sites per vector access
     // Exchange of the pair that straddles two warps of a line: entry b (b = the block's warp index
@@ -488,10 +496,19 @@ line_kernel(const __grid_constant__ LineParams<T> p) {
                 __syncwarp();
                 if (is_first) mbar_arrive(bar);
             }
-            up.re = __shfl_sync(0xffffffffu, M.s[NS - 1].re, up_src);
-            up.im = __shfl_sync(0xffffffffu, M.s[NS - 1].im, up_src);
-            dn.re = __shfl_sync(0xffffffffu, M.s[0].re, dn_src);
-            dn.im = __shfl_sync(0xffffffffu, M.s[0].im, dn_src);
+            if (MW) {
+                // neighbouring lanes by a constant distance (no index arithmetic in the loop);
+                // lanes 0 / 31 get their own value back and take the other warp's in xend
+                up.re = __shfl_up_sync(0xffffffffu, M.s[NS - 1].re, 1);
+                up.im = __shfl_up_sync(0xffffffffu, M.s[NS - 1].im, 1);
+                dn.re = __shfl_down_sync(0xffffffffu, M.s[0].re, 1);
+                dn.im = __shfl_down_sync(0xffffffffu, M.s[0].im, 1);
+            } else {
+                up.re = __shfl_sync(0xffffffffu, M.s[NS - 1].re, up_src);
+                up.im = __shfl_sync(0xffffffffu, M.s[NS - 1].im, up_src);
+                dn.re = __shfl_sync(0xffffffffu, M.s[0].re, dn_src);
+                dn.im = __shfl_sync(0xffffffffu, M.s[0].im, dn_src);
+            }
         };
         auto xend = [&](Cx<T>& up, Cx<T>& dn) {
             if (MW) {
@@ -1156,7 +1173,7 @@ int launch_line(const LineParams<T>& p, cudaStream_t st) {
     // several warps per line: the grid strides over the lines (barrier state lives in the block)
     int64_t blocks = groups;
     if (MW) {
-        const int64_t resident = (int64_t)sm_count() * (512 / threads);
+        const int64_t resident = (int64_t)sm_count() * ((sizeof(T) * NS >= 256 ? 256 : 512) / threads);
         if (blocks > resident) blocks = resident;
     }
     line_kernel<T, NS, EDGE, COL, MW><<<(unsigned)blocks, threads, 0, st>>>(p);
@@ -1182,6 +1199,13 @@ int launch_line_t(const LineParams<T>& p, int ns, bool edge, bool col, cudaStrea
         case 16: return launch_line_ns<T, 16>(p, edge, col, st);
         case 32:
             if constexpr (sizeof(T) == 4) return launch_line_ns<T, 32>(p, edge, col, st);
+            break;
+        case 64:      // rows of fp32, several warps per line only (launch_lines)
+            if constexpr (sizeof(T) == 4) {
+                if (!col && p.n_warps > 1)
+                    return edge ? launch_line<T, 64, true, false, true>(p, st)
+                                : launch_line<T, 64, false, false, true>(p, st);
+            }
     }
     set_error("axis: no line kernel for this extent");
     return TS_EUNSUPPORTED;
@@ -1260,8 +1284,21 @@ int launch_lines(const LineGeom& g, int dtype, LineParams<T>& p, T* re, T* im, c
             return launch_tline<T>(p, ts_.ns, !g.periodic, st);
         }
     }
-    const LineShape sh = line_shape(g.n_sites, dtype);
+    LineShape sh = line_shape(g.n_sites, dtype);
     if (!sh.ok()) { set_error("axis: line does not fit a thread block"); return TS_EUNSUPPORTED; }
+    // long fp32 rows: 64 sites per lane and half the warps -- the per-sub-step cost of the exchange
+    // (publish, arrive, wait, pick up: ~45 instructions per warp) is spread over twice the sites,
+    // at 255 registers, i.e. 8 warps per SM.  Taken where those 8 warps are whole lines of 2, 4 or
+    // 8 warps and it measured faster (200 sub-steps, rows only, ms, 32 -> 64 sites per lane):
+    // 4096^2 0.600 -> 0.580 / closed 0.648 -> 0.582, 8192^2 2.35 -> 2.30 / closed 2.60 -> 2.31,
+    // 16384^2 closed 9.51 -> 9.06; NOT for periodic rows of 16384 (one line of 8 warps per SM:
+    // 8.53 -> 8.86) nor where the warps do not fill the SM (12288: 1.76 -> 2.12).
+    static const bool ns64 = getenv("TS_PROBE_NO_NS64") == nullptr;
+    if (ns64 && !g.col && dtype == TS_F32 && sh.ns == 32 &&
+        (sh.warps == 4 || sh.warps == 8 || (sh.warps == 16 && !g.periodic))) {
+        sh.ns = 64;
+        sh.warps /= 2;
+    }
     p.n_lanes = sh.lanes;
     p.n_warps = sh.warps;
     if (sh.warps == 1) {

@@ -51,18 +51,19 @@ def test_resident_lines(dtype, boundary, idx, n_steps):
     assert info["chain_x"] == n_steps and info["chain_y"] == n_steps
 
 
-# lines shared by several warps of a block (2048 = 2 x 32 x 32, 1152 = 9 x 32 x 4, ...), rows that
+# lines shared by several warps of a block (2048 = 2 x 32 x 32, 1152 = 9 x 32 x 4, 4096 / 8192 /
+# closed 16384 in fp32 = 2 / 4 / 8 warps of 64 sites per lane, ...), rows that
 # fit no block and are cut into windows with a halo (1056 = 33 x 32, 20480, 528, 12288), columns
 # that are pipelined (130, 1100, 66 rows: no lane layout divides them)
 LONG = {"f32": [(2048, 128), (1152, 200), (64, 2048), (1280, 130), (3072, 1100), (4096, 66),
-                (1056, 200), (20480, 66), (16384, 16)],
+                (1056, 200), (20480, 66), (16384, 16), (8192, 12)],
         "f64": [(1024, 128), (576, 200), (64, 1024), (640, 130), (1536, 1100), (528, 200),
                 (12288, 66), (8192, 16)]}
 
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 @pytest.mark.parametrize("boundary", ["closed", "periodic"])
-@pytest.mark.parametrize("idx", range(9))
+@pytest.mark.parametrize("idx", range(10))
 @pytest.mark.parametrize("chain", [0, 4, 7, 16, 24])
 def test_multi_warp_lines_windowed_rows_and_pipelined_columns(dtype, boundary, idx, chain):
     if idx >= len(LONG[dtype]):
