@@ -435,9 +435,13 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
     // warp) or beyond S = 2 (255 registers) two, everything else three
     const bool planes = any_pot && !(any_sep && use_stream);
     const int bpsm = (L.dtype == TS_F64 && (planes || S > 2)) ? 2 : 3;
-    const int seg = plan->opt_seg ? (int)plan->opt_seg
-                    : use_stream ? ts::stream_default_seg_rows(L, S, bpsm)
-                                 : ts::fused_default_seg_rows(L, S, bpsm);
+    // an explicit "seg_rows" means equal segments; by default the tile kernel's edge warps get
+    // shorter ones (stream_default_seg)
+    const ts::SegShape sseg = plan->opt_seg ? ts::SegShape{(int)plan->opt_seg, 0}
+                                            : ts::stream_default_seg(L, S, bpsm);
+    const int seg = use_stream ? sseg.rows
+                               : plan->opt_seg ? (int)plan->opt_seg
+                                               : ts::fused_default_seg_rows(L, S, bpsm);
     plan->info_variant = use_stream ? 2 : 1;
     void* cur_re = psi_re; void* cur_im = psi_im;
     void* nxt_re = plan->scratch_re; void* nxt_im = plan->scratch_im;
@@ -456,7 +460,7 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
         }
         ts::timer_begin(tm, use_stream ? ts::kKindStream : ts::kKindFused, st);
         if (use_stream)
-            rc = ts::stream_pass(L, cur_re, cur_im, nxt_re, nxt_im, subs, ph, s, seg,
+            rc = ts::stream_pass(L, cur_re, cur_im, nxt_re, nxt_im, subs, ph, s, sseg,
                                  (int)plan->opt_slots, st);
         else
             rc = ts::fused_pass(L, cur_re, cur_im, nxt_re, nxt_im, subs[0], ph.planes, s, seg, st);
@@ -608,8 +612,9 @@ int ts_slab_pass(ts_plan* plan, const void* src_re, const void* src_im, void* ds
     if (rc != TS_OK) return rc;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
     const ts::Peers peers{up_re, up_im, up_rows, dn_re, dn_im, dn_rows};
-    const int seg = plan->opt_seg ? (int)plan->opt_seg : ts::stream_default_seg_rows(L, n_sub, 3);
-    rc = ts::stream_pass(L, src_re, src_im, dst_re, dst_im, subs, ph, n_sub, seg,
+    // slabs: equal segments (the cut rows of a slab are not lattice edges)
+    const int seg = plan->opt_seg ? (int)plan->opt_seg : ts::stream_default_seg(L, n_sub, 3).rows;
+    rc = ts::stream_pass(L, src_re, src_im, dst_re, dst_im, subs, ph, n_sub, ts::SegShape{seg, 0},
                          (int)plan->opt_slots, st, &peers);
     if (rc != TS_OK) return rc;
     plan->info_fused = 1; plan->info_fuse = n_sub; plan->info_passes = 1; plan->info_launches = 1;

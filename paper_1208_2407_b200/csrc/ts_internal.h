@@ -114,11 +114,17 @@ bool stream_supported(const LatticeDesc& L, const StepCoef& c);
 int stream_max_steps(const LatticeDesc& L, bool pot);   // 6 for fp32 without potential, else 4
 int stream_default_steps_sep(const LatticeDesc& L);     // sub-steps per pass, separable phase
 int stream_default_slots(const LatticeDesc& L, int S, bool pot);
-int stream_default_seg_rows(const LatticeDesc& L, int S, int blocks_per_sm = 3);
+// Segment heights of one pass: `rows` for warps that run the plain loop, `edge` (<= rows; 0: as
+// rows) for warps that run the closed-edge variant of it (x-edge strips, first / last segment of
+// a lattice closed in y), which costs ~8 % more per row.
+struct SegShape {
+    int rows, edge;
+};
+SegShape stream_default_seg(const LatticeDesc& L, int S, int blocks_per_sm = 3);
 // One pass: dst <- U2(subs[S-1]) ... U2(subs[0]) src; the S sub-steps may have different angles
 // (fourth-order step, Eq. 4) but share one potential-phase array.
 int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
-                void* dst_im, const StepCoef* subs, const Phase& ph, int S, int seg_rows, int nst,
+                void* dst_im, const StepCoef* subs, const Phase& ph, int S, SegShape seg, int nst,
                 cudaStream_t st, const Peers* peers = nullptr);
 // pot[2][ny][nx] <- px (x) py: the separable factors written out for paths that take planes
 int expand_separable(const LatticeDesc& L, const void* px, const void* py, void* pot,

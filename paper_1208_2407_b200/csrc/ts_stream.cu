@@ -58,6 +58,11 @@ struct StreamParams {
     int py_off, py_n, py_wrap;   // separable phase: global row of local row 0, global height, wrap
     int nx, ny;
     int n_strips, wi, halo, seg_rows, n_seg;
+    // warps that run the closed-edge variant of the loop get shorter segments (seg_edge <=
+    // seg_rows): the n_xe x-edge strips (first / last strip of a lattice closed in x; 0, 1 or 2)
+    // are cut into n_seg_x segments of seg_edge rows; with y_short the first and the last segment
+    // of every other strip are seg_edge rows high and the n_seg - 2 between them seg_rows
+    int seg_edge, n_seg_x, n_xe, y_short;
     int nst;        // ring slots per warp (state row pairs)
     int nph;        // with phase planes: slots of the separate phase ring (>= prefetch + S + 1)
     // tangents of the sweeps of the S chained sub-steps of this pass (angles may differ from
@@ -242,10 +247,27 @@ stream_kernel(const StreamParams<T> p) {
     // n_strips is not a multiple of kWarps (4096^2 at S = 3: 37 strips, 48 segments = 1776 warps,
     // exactly one wave of 444 blocks; with a grid of (10, 44) three warps in forty were empty and
     // every warp had 8 more rows).  Warps share nothing (own ring, own barriers).
+    // Warps that run the closed-edge variant (about 8 % more per row) would end every pass late:
+    // they get shorter segments (StreamParams::seg_edge), the x-edge strips first in the numbering.
     const int wid = blockIdx.x * kWarps + warp;
-    const int segi = wid / p.n_strips;
-    const int strip = wid - segi * p.n_strips;
-    if (segi >= p.n_seg) return;
+    int segi, strip;
+    bool x_short = false;
+    {
+        const int we = p.n_xe * p.n_seg_x;
+        if (wid < we) {
+            const int k = wid / p.n_seg_x;
+            segi = wid - k * p.n_seg_x;
+            strip = k == 0 ? 0 : p.n_strips - 1;
+            x_short = true;
+        } else {
+            const int ni = p.n_strips - p.n_xe;
+            if (ni <= 0) return;
+            const int w2 = wid - we;
+            segi = w2 / ni;
+            strip = (p.n_xe > 0 ? 1 : 0) + (w2 - segi * ni);
+            if (segi >= p.n_seg) return;
+        }
+    }
     const int NST = p.nst;
     const int NPH = POT ? p.nph : 0;
     const int DIST = NST - R;                 // prefetch distance in iterations
@@ -282,8 +304,21 @@ stream_kernel(const StreamParams<T> p) {
     const uint32_t slot_tx = NROW * (bytes_a + bytes_b);
     const uint32_t dst_a = off_a * sizeof(T), dst_b = bytes_a;
 
-    const int y_out0 = segi * p.seg_rows;
-    const int y_out1 = min(y_out0 + p.seg_rows, p.ny);
+    int y_out0, y_out1;
+    if (x_short) {
+        y_out0 = segi * p.seg_edge;
+        y_out1 = min(y_out0 + p.seg_edge, p.ny);
+    } else if (p.y_short) {
+        if (segi == 0) { y_out0 = 0; y_out1 = p.seg_edge; }
+        else if (segi == p.n_seg - 1) { y_out0 = p.ny - p.seg_edge; y_out1 = p.ny; }
+        else {
+            y_out0 = p.seg_edge + (segi - 1) * p.seg_rows;
+            y_out1 = min(y_out0 + p.seg_rows, p.ny - p.seg_edge);
+        }
+    } else {
+        y_out0 = segi * p.seg_rows;
+        y_out1 = min(y_out0 + p.seg_rows, p.ny);
+    }
     const int y_in0 = y_out0 - 2 * S;
     // even, so that the two-iteration loop body has no conditional half (the extra iteration only
     // feeds the pipeline; its output row pair lies beyond the segment and is not stored)
@@ -468,7 +503,8 @@ int launch(const StreamParams<T>& p, cudaStream_t st) {
                                          (int)smem));
         if (dev >= 0 && dev < kMaxDevices) configured[dev].store(smem, std::memory_order_relaxed);
     }
-    dim3 grid((unsigned)(((int64_t)p.n_strips * p.n_seg + kWarps - 1) / kWarps));
+    const int64_t n_warps = (int64_t)p.n_xe * p.n_seg_x + (int64_t)(p.n_strips - p.n_xe) * p.n_seg;
+    dim3 grid((unsigned)((n_warps + kWarps - 1) / kWarps));
     // programmatic dependent launch pays where launch latency and the prologue are a visible part
     // of a pass, i.e. for grids of at most one wave (1024^2 +12 %, 2048^2 +17 %, 4096^2 +0-2 %);
     // on many-wave grids the next pass's blocks then start in lockstep and a 16384^2 pass gets
@@ -512,7 +548,7 @@ int launch_s(const StreamParams<T>& p, int pm, int bnd, cudaStream_t st) {
 
 template <typename T>
 int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T* dst_im,
-           const StepCoef* subs, const Phase& ph, int S, int seg_rows, int nst, cudaStream_t st,
+           const StepCoef* subs, const Phase& ph, int S, SegShape seg, int nst, cudaStream_t st,
            const Peers* peers) {
     StreamParams<T> p;
     p.up_re = p.up_im = p.dn_re = p.dn_im = nullptr;
@@ -542,8 +578,21 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
     p.halo = (2 * S + 3) / 4 * 4;
     p.wi = kStripSites - 2 * p.halo;
     p.n_strips = (int)((L.nx + p.wi - 1) / p.wi);
-    p.seg_rows = seg_rows;
-    p.n_seg = (int)((L.ny + seg_rows - 1) / seg_rows);
+    p.seg_rows = seg.rows;
+    p.n_seg = (int)((L.ny + seg.rows - 1) / seg.rows);
+    p.seg_edge = seg.rows; p.n_seg_x = 0; p.n_xe = 0; p.y_short = 0;
+    if (seg.edge > 0 && seg.edge < seg.rows) {
+        p.seg_edge = seg.edge;
+        if (!L.periodic_x) {
+            p.n_xe = p.n_strips < 2 ? p.n_strips : 2;
+            p.n_seg_x = (int)((L.ny + seg.edge - 1) / seg.edge);
+        }
+        // first and last segment short: only where rows are left for a segment between them
+        if (!L.periodic_y && L.ny >= 2 * (int64_t)seg.edge + 2) {
+            p.y_short = 1;
+            p.n_seg = 2 + (int)((L.ny - 2 * seg.edge + seg.rows - 1) / seg.rows);
+        }
+    }
     // state ring: prefetch distance + 1 slots; phase ring (planes only): prefetch + S + 1
     if (nst <= 0) nst = stream_default_slots(L, S, pot != nullptr);   // separable: as without
     if (nst < 2) nst = 2;
@@ -633,16 +682,16 @@ int pass_t(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re, T*
 
 #if TS_STREAM_TU == 0 || TS_STREAM_TU == 64
 int stream_pass_f64(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
-                    void* dst_im, const StepCoef* subs, const Phase& ph, int S, int seg_rows,
+                    void* dst_im, const StepCoef* subs, const Phase& ph, int S, SegShape seg,
                     int nst, cudaStream_t st, const Peers* peers) {
     return pass_t<double>(L, (const double*)src_re, (const double*)src_im, (double*)dst_re,
-                          (double*)dst_im, subs, ph, S, seg_rows, nst, st, peers);
+                          (double*)dst_im, subs, ph, S, seg, nst, st, peers);
 }
 #endif
 
 #if TS_STREAM_TU == 0 || TS_STREAM_TU == 32
 int stream_pass_f64(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
-                    void* dst_im, const StepCoef* subs, const Phase& ph, int S, int seg_rows,
+                    void* dst_im, const StepCoef* subs, const Phase& ph, int S, SegShape seg,
                     int nst, cudaStream_t st, const Peers* peers);
 
 bool stream_supported(const LatticeDesc& L, const StepCoef& c) {
@@ -676,11 +725,15 @@ int stream_default_slots(const LatticeDesc& L, int S, bool pot) {
     return L.dtype == TS_F32 ? 8 : 6;
 }
 
-int stream_default_seg_rows(const LatticeDesc& L, int S, int blocks_per_sm) {
-    // As fused_default_seg_rows (a segment costs seg/2 + 2S iterations; whole waves, since a grid
-    // of 1.1 waves costs two), but counted in WARPS: the kernel deals (strip, segment) pairs to
-    // warps without gaps, so the machine holds 148 * blocks_per_sm * kWarps of them per wave
-    // whatever n_strips is.
+SegShape stream_default_seg(const LatticeDesc& L, int S, int blocks_per_sm) {
+    // As fused_default_seg_rows (a segment of r rows costs r/2 + 2S + 1 iterations; whole waves,
+    // since a grid of 1.1 waves costs two), but counted in WARPS: the kernel deals (strip, segment)
+    // pairs to warps without gaps, so the machine holds 148 * blocks_per_sm * kWarps of them per
+    // wave whatever n_strips is.  Warps at a closed edge run the edge variant of the loop, which
+    // costs kEdgeCost per row of the plain one (4096^2 at S = 3: 76.7 us per pass periodic, 82.6
+    // closed with equal segments): their segments are shortened by that factor, and the smallest
+    // plain height whose warp count still fits the waves is taken.
+    constexpr double kEdgeCost = 1.08;
     const int halo = (2 * S + 3) / 4 * 4;
     const int64_t strips = (L.nx + (kStripSites - 2 * halo) - 1) / (kStripSites - 2 * halo);
     const int64_t slots = 148 * (int64_t)(blocks_per_sm > 0 ? blocks_per_sm : 3) * kWarps;
@@ -695,20 +748,43 @@ int stream_default_seg_rows(const LatticeDesc& L, int S, int blocks_per_sm) {
     if (r > cap) r = cap;
     if (r < 8) r = 8;     // small lattices: parallelism over warm-up redundancy
     if (r > L.ny) r = L.ny;
-    return (int)r;
+    SegShape out{(int)r, 0};
+    const bool closed = !L.periodic_x || !L.periodic_y;
+    static const bool no_short = getenv("TS_PROBE_NO_SHORT_EDGE") != nullptr;   // tuning probe only
+    if (!closed || no_short || r < 32 || L.ny < 4 * r) return out;
+    auto edge_of = [&](int64_t h) {
+        int64_t e = (int64_t)(2.0 * ((h / 2 + 2 * S + 1) / kEdgeCost - (2 * S + 1)));
+        e -= e % 2;
+        if (e < 8) e = 8;
+        return e < h ? e : h;
+    };
+    auto warps_of = [&](int64_t h, int64_t e) {
+        const int64_t n_xe = L.periodic_x ? 0 : (strips < 2 ? strips : 2);
+        const int64_t seg_x = (L.ny + e - 1) / e;
+        int64_t seg_i = (L.ny + h - 1) / h;
+        if (!L.periodic_y) seg_i = 2 + (L.ny - 2 * e + h - 1) / h;
+        return n_xe * seg_x + (strips - n_xe) * seg_i;
+    };
+    // the equal-height choice r fits by construction; taller plain segments make room for the
+    // extra (short) edge segments
+    for (int64_t h = r; h <= cap; h += 2) {
+        const int64_t e = edge_of(h);
+        if (warps_of(h, e) <= waves * slots) return SegShape{(int)h, (int)e};
+    }
+    return out;
 }
 
 int stream_pass(const LatticeDesc& L, const void* src_re, const void* src_im, void* dst_re,
-                void* dst_im, const StepCoef* subs, const Phase& ph, int S, int seg_rows, int nst,
+                void* dst_im, const StepCoef* subs, const Phase& ph, int S, SegShape seg, int nst,
                 cudaStream_t st, const Peers* peers) {
-    if (seg_rows <= 0 || seg_rows % 2) {
-        set_error("stream_pass: seg_rows must be positive and even");
+    if (seg.rows <= 0 || seg.rows % 2 || seg.edge < 0 || seg.edge % 2 || seg.edge > seg.rows) {
+        set_error("stream_pass: segment heights must be positive and even, edge <= rows");
         return TS_EINVAL;
     }
     if (L.dtype == TS_F32)
         return pass_t<float>(L, (const float*)src_re, (const float*)src_im, (float*)dst_re,
-                             (float*)dst_im, subs, ph, S, seg_rows, nst, st, peers);
-    return stream_pass_f64(L, src_re, src_im, dst_re, dst_im, subs, ph, S, seg_rows, nst, st,
+                             (float*)dst_im, subs, ph, S, seg, nst, st, peers);
+    return stream_pass_f64(L, src_re, src_im, dst_re, dst_im, subs, ph, S, seg, nst, st,
                            peers);
 }
 #endif

@@ -175,3 +175,43 @@ def test_slab_pass_argument_errors():
     with pytest.raises(TsError):
         per.slab_pass(a, b, None, None, [c])                 # slab plans are closed in y
     per.destroy()
+
+
+@pytest.mark.parametrize("bx,by,nx,ny,dtype,with_pot", [
+    ("closed", "closed", 700, 20000, "f32", True),       # S = 3: x-edge strips and y-edge segments short
+    ("closed", "closed", 700, 20000, "f32", False),      # S = 6 on the tile kernel (variant 2)
+    ("periodic", "closed", 512, 24000, "f32", True),     # no x-edge strips, y-edge segments short
+    ("closed", "closed", 100, 60000, "f32", True),       # one strip: every warp is an edge warp
+    ("closed", "closed", 200, 30000, "f32", True),       # two strips, both x-edge
+    ("closed", "closed", 600, 12000, "f64", True),       # two blocks per SM
+    ("periodic", "periodic", 512, 24000, "f32", True),   # nothing closed: equal segments
+])
+def test_default_segments_on_tall_lattices(bx, by, nx, ny, dtype, with_pot):
+    """DEFAULT segment heights of the tile kernel on lattices tall enough that the warps at a
+    closed edge get shorter segments than the others (ts_stream.cu: stream_default_seg; the
+    other tests force equal segments with the seg_rows option or are too small for the split):
+    every element against the oracle."""
+    import torch
+    from paper_1208_2407_b200.binding import Plan
+    dev = torch.device("cuda:0")
+    re, im, pot = G.random_inputs(nx, ny, dtype, 7 * nx + ny, with_pot)
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    plan = Plan(nx, ny, tdt, bx, by)
+    plan.set_option("path", 2); plan.set_option("variant", 2)
+    dre, dim = torch.from_numpy(re).to(dev), torch.from_numpy(im).to(dev)
+    dpot = None if pot is None else torch.from_numpy(pot).to(dev)
+    n = 7
+    n0 = plan.norm(dre, dim)
+    plan.evolve(dre, dim, *coeffs(0.3), pot_phase=dpot, n_steps=n)
+    torch.cuda.synchronize()
+    n1 = plan.norm(dre, dim)
+    assert plan.info("fused") == 1 and plan.info("variant") == 2
+    assert plan.info("seg_rows") >= 32, plan.info("seg_rows")
+    wre, wim = re.astype(np.float64), im.astype(np.float64)
+    p64 = None if pot is None else (pot[0].astype(np.float64), pot[1].astype(np.float64))
+    oracle.evolve_xy(wre, wim, *coeffs(0.3), pot=p64, periodic_x=bx == "periodic",
+                     periodic_y=by == "periodic", n_steps=n)
+    err = max(np.abs(dre.cpu().numpy() - wre).max(), np.abs(dim.cpu().numpy() - wim).max())
+    assert err <= TIGHT[dtype] * 2, err
+    assert abs(n1 / n0 - 1) < (1e-5 if dtype == "f32" else 1e-12)
+    plan.destroy()
