@@ -476,7 +476,7 @@ def run_gpu(args):
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3,
                 "api": e2e_api,
-                "note": "host<->device copies and compute are serialised inside the call"},
+                "note": "PCIe-bound: without a potential the planes go up in 8 row pieces and the row chain of a piece runs under the upload of the next; the column passes and the download are serial"},
         "gpu_launches": info["launches"] * args.steps,
         "roofline": roof,
         "cpu_baseline": time_oracle(args.config, args.cpu_budget, full_ok=True),

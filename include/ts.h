@@ -242,6 +242,10 @@ int ts_norm_static(int dtype, const void* psi_re, const void* psi_im, int64_t n_
  * ts_evolve_host -- the same operation for HOST-resident planes (pageable or pinned): copies
  * psi (and pot_phase when given) to plan-owned device buffers, runs ts_evolve, copies psi
  * back, and synchronises.  This is the end-to-end entry measured by bench.py's "e2e".
+ * Large lattices without a potential go up in 8 pieces of rows on a second plan-owned stream; where
+ * the rows are evolved as resident lines (the axis-split path) the row chain of a piece runs while
+ * the next piece is still on the bus, every other path waits for the last piece.  The result is
+ * bit-identical to ts_evolve on device planes.  On an error nothing is left running.
  */
 int ts_evolve_host(ts_plan* plan, void* psi_re_host, void* psi_im_host,
                    double a_half, double b_half, double a_full, double b_full,

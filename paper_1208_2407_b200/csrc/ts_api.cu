@@ -56,6 +56,11 @@ struct ts_plan {
     void* host_pot;
     void* sep_pot;            // separable phase written out as planes (paths without mode 2)
     cudaStream_t own_stream;
+    // ts_evolve_host: the planes go up in kFeedPieces pieces on copy_stream, one event per piece;
+    // feed is set for the duration of that call only
+    cudaStream_t copy_stream;
+    cudaEvent_t feed_ev[8];
+    const ts::RowFeed* feed;
     // options
     int64_t opt_path, opt_fuse, opt_seg, opt_variant, opt_slots, opt_chain;
     // info on the last ts_evolve
@@ -190,6 +195,9 @@ int ts_plan_destroy(ts_plan* plan) {
     cudaFree(plan->host_pot);
     cudaFree(plan->sep_pot);
     if (plan->own_stream) cudaStreamDestroy(plan->own_stream);
+    if (plan->copy_stream) cudaStreamDestroy(plan->copy_stream);
+    for (cudaEvent_t e : plan->feed_ev)
+        if (e) cudaEventDestroy(e);
     delete plan->timer;
     delete plan;
     return TS_OK;
@@ -365,6 +373,9 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
         }
     }
 
+    // host-fed planes (ts_evolve_host): only the axis-split path starts on a part of the rows
+    if (plan->feed && !use_axis && plan->feed->n > 0)
+        TS_CUDA_TRY(cudaStreamWaitEvent(st, plan->feed->ready[plan->feed->n - 1], 0));
     if (use_axis) {
         if (ts::axis_needs_scratch(L)) {
             rc = ensure_alloc(&plan->scratch_re, plane_bytes);
@@ -374,7 +385,7 @@ int evolve_pattern(ts_plan* plan, void* psi_re, void* psi_im, const SubStep* pat
         ts::AxisInfo ai;
         rc = ts::axis_evolve(L, psi_re, psi_im, plan->scratch_re, plan->scratch_im, axis_pat, period,
                              n_sub, (int)plan->opt_chain, (int)plan->opt_seg, (int)plan->opt_slots,
-                             st, &ai, tm);
+                             st, &ai, tm, plan->feed);
         plan->info_launches = ai.launches;
         if (rc != TS_OK) return rc;
         plan->info_fused = 1; plan->info_passes = ai.passes; plan->info_seg = ai.seg_rows;
@@ -744,14 +755,66 @@ int ts_evolve_host(ts_plan* plan, void* re_h, void* im_h, double a_half, double 
     if (!plan->own_stream)
         TS_CUDA_TRY(cudaStreamCreateWithFlags(&plan->own_stream, cudaStreamNonBlocking));
     cudaStream_t st = plan->own_stream;
-    TS_CUDA_TRY(cudaMemcpyAsync(plan->host_re, re_h, plane_bytes, cudaMemcpyHostToDevice, st));
-    TS_CUDA_TRY(cudaMemcpyAsync(plan->host_im, im_h, plane_bytes, cudaMemcpyHostToDevice, st));
-    if (pot_h)
-        TS_CUDA_TRY(cudaMemcpyAsync(plan->host_pot, pot_h, 2 * plane_bytes,
-                                    cudaMemcpyHostToDevice, st));
-    rc = ts_evolve(plan, plan->host_re, plan->host_im, a_half, b_half, a_full, b_full,
-                   pot_h ? plan->host_pot : nullptr, n_steps, st);
-    if (rc != TS_OK) return rc;
+    // Without a potential the step factorises into a row chain and a column chain (ts_axis.cu) and
+    // rows are independent lines: the planes go up in pieces on a second stream and the row chain
+    // of a piece runs while the next piece is on the bus (C4: the 8.6 ms of the row chain hidden
+    // behind the 39 ms of the upload).  Paths that need the whole lattice wait for the last piece.
+    constexpr int kFeedPieces = 8;
+    const bool pieces = !pot_h && plan->nz == 1 && plan->L.ny >= 64 * kFeedPieces &&
+                        plane_bytes >= (size_t(8) << 20);
+    if (pieces) {
+        if (!plan->copy_stream)
+            TS_CUDA_TRY(cudaStreamCreateWithFlags(&plan->copy_stream, cudaStreamNonBlocking));
+        for (int k = 0; k < kFeedPieces; ++k)
+            if (!plan->feed_ev[k])
+                TS_CUDA_TRY(cudaEventCreateWithFlags(&plan->feed_ev[k], cudaEventDisableTiming));
+        cudaStream_t cs = plan->copy_stream;
+        int64_t y_end[kFeedPieces];
+        const size_t row_bytes = (size_t)plan->L.nx * plan->elem;
+        int64_t y0 = 0;
+        for (int k = 0; k < kFeedPieces; ++k) {
+            int64_t y1 = plan->L.ny * (k + 1) / kFeedPieces;
+            y1 -= y1 % 2;
+            if (k == kFeedPieces - 1) y1 = plan->L.ny;
+            y_end[k] = y1;
+            const size_t off = (size_t)y0 * row_bytes, nb = (size_t)(y1 - y0) * row_bytes;
+            cudaError_t e = cudaMemcpyAsync((char*)plan->host_re + off, (const char*)re_h + off, nb,
+                                            cudaMemcpyHostToDevice, cs);
+            if (e == cudaSuccess)
+                e = cudaMemcpyAsync((char*)plan->host_im + off, (const char*)im_h + off, nb,
+                                    cudaMemcpyHostToDevice, cs);
+            if (e == cudaSuccess) e = cudaEventRecord(plan->feed_ev[k], cs);
+            if (e != cudaSuccess) {
+                cudaStreamSynchronize(cs);
+                return ts::cuda_fail(e, "ts_evolve_host: upload");
+            }
+            y0 = y1;
+        }
+        const ts::RowFeed feed{kFeedPieces, y_end, plan->feed_ev};
+        plan->feed = &feed;
+        rc = ts_evolve(plan, plan->host_re, plan->host_im, a_half, b_half, a_full, b_full, nullptr,
+                       n_steps, st);
+        plan->feed = nullptr;
+        if (rc != TS_OK) {
+            cudaStreamSynchronize(cs);
+            cudaStreamSynchronize(st);
+            return rc;
+        }
+        // (a call of zero steps enqueues nothing that waits for the upload)
+        TS_CUDA_TRY(cudaStreamWaitEvent(st, plan->feed_ev[kFeedPieces - 1], 0));
+    } else {
+        TS_CUDA_TRY(cudaMemcpyAsync(plan->host_re, re_h, plane_bytes, cudaMemcpyHostToDevice, st));
+        TS_CUDA_TRY(cudaMemcpyAsync(plan->host_im, im_h, plane_bytes, cudaMemcpyHostToDevice, st));
+        if (pot_h)
+            TS_CUDA_TRY(cudaMemcpyAsync(plan->host_pot, pot_h, 2 * plane_bytes,
+                                        cudaMemcpyHostToDevice, st));
+        rc = ts_evolve(plan, plan->host_re, plan->host_im, a_half, b_half, a_full, b_full,
+                       pot_h ? plan->host_pot : nullptr, n_steps, st);
+        if (rc != TS_OK) {
+            cudaStreamSynchronize(st);      // the uploads still read the caller's planes
+            return rc;
+        }
+    }
     TS_CUDA_TRY(cudaMemcpyAsync(re_h, plan->host_re, plane_bytes, cudaMemcpyDeviceToHost, st));
     TS_CUDA_TRY(cudaMemcpyAsync(im_h, plan->host_im, plane_bytes, cudaMemcpyDeviceToHost, st));
     TS_CUDA_TRY(cudaStreamSynchronize(st));

@@ -1612,7 +1612,8 @@ int axis_default_chain(const LatticeDesc& L) {
 template <typename T>
 static int axis_evolve_t(const LatticeDesc& L, T* psi_re, T* psi_im, T* scr_re, T* scr_im,
                          const StepCoef* pat, int period, int64_t n_sub, int chain, int seg_rows,
-                         int nst, cudaStream_t st, AxisInfo* info, LaunchTimer* tm) {
+                         int nst, cudaStream_t st, AxisInfo* info, LaunchTimer* tm,
+                         const RowFeed* feed) {
     T* cur_re = psi_re; T* cur_im = psi_im;
     T* nxt_re = scr_re; T* nxt_im = scr_im;
     auto flip = [&]() {
@@ -1666,13 +1667,37 @@ static int axis_evolve_t(const LatticeDesc& L, T* psi_re, T* psi_im, T* scr_re, 
     // ---- rows
     if (x_res) {
         const bool flip_here = odd_flips;
-        timer_begin(tm, kKindLineRows, st);
-        rc = line_pass<T>(L, cur_re, cur_im, pat, period, n_sub, false, st,
-                          flip_here ? nxt_re : nullptr, flip_here ? nxt_im : nullptr);
-        timer_end(tm, st);
-        if (rc != TS_OK) return rc;
+        if (feed && feed->n > 1) {
+            // rows are independent lines: one launch per piece of the feed, each after its copy
+            int64_t y0 = 0;
+            for (int k = 0; k < feed->n; ++k) {
+                const int64_t y1 = feed->y_end[k];
+                TS_CUDA_TRY(cudaStreamWaitEvent(st, feed->ready[k], 0));
+                if (y1 > y0) {
+                    LatticeDesc Lk = L;
+                    Lk.ny = y1 - y0;
+                    const int64_t off = y0 * L.nx;
+                    timer_begin(tm, kKindLineRows, st);
+                    rc = line_pass<T>(Lk, cur_re + off, cur_im + off, pat, period, n_sub, false, st,
+                                      flip_here ? nxt_re + off : nullptr,
+                                      flip_here ? nxt_im + off : nullptr);
+                    timer_end(tm, st);
+                    if (rc != TS_OK) return rc;
+                    ++info->launches;
+                }
+                y0 = y1;
+            }
+        } else {
+            if (feed && feed->n == 1) TS_CUDA_TRY(cudaStreamWaitEvent(st, feed->ready[0], 0));
+            timer_begin(tm, kKindLineRows, st);
+            rc = line_pass<T>(L, cur_re, cur_im, pat, period, n_sub, false, st,
+                              flip_here ? nxt_re : nullptr, flip_here ? nxt_im : nullptr);
+            timer_end(tm, st);
+            if (rc != TS_OK) return rc;
+            ++info->launches;
+        }
         if (flip_here) flip();
-        ++info->passes; ++info->launches;
+        ++info->passes;
         info->chain_x = n_sub;
     } else {
         for (int64_t i = 0; i < n_sub; i += x_chain) {
@@ -1737,16 +1762,22 @@ bool axis_needs_scratch(const LatticeDesc& L) {
 
 int axis_evolve(const LatticeDesc& L, void* psi_re, void* psi_im, void* scr_re, void* scr_im,
                 const StepCoef* pat, int period, int64_t n_sub, int chain, int seg_rows, int nst,
-                cudaStream_t st, AxisInfo* info, LaunchTimer* tm) {
+                cudaStream_t st, AxisInfo* info, LaunchTimer* tm, const RowFeed* feed) {
     if (chain <= 0) chain = axis_default_chain(L);
+    if (feed && !axis_takes_feed(L)) {       // windowed rows: whole lattice first
+        if (feed->n > 0) TS_CUDA_TRY(cudaStreamWaitEvent(st, feed->ready[feed->n - 1], 0));
+        feed = nullptr;
+    }
     if (L.dtype == TS_F32)
         return axis_evolve_t<float>(L, (float*)psi_re, (float*)psi_im, (float*)scr_re,
                                     (float*)scr_im, pat, period, n_sub, chain, seg_rows, nst, st,
-                                    info, tm);
+                                    info, tm, feed);
     return axis_evolve_t<double>(L, (double*)psi_re, (double*)psi_im, (double*)scr_re,
                                  (double*)scr_im, pat, period, n_sub, chain, seg_rows, nst, st,
-                                 info, tm);
+                                 info, tm, feed);
 }
+
+bool axis_takes_feed(const LatticeDesc& L) { return line_shape(L.nx, L.dtype).ok(); }
 
 
 // ---- three-dimensional lattices (ts_internal.h) -------------------------------------------------------

@@ -139,6 +139,14 @@ int fused_default_steps(const LatticeDesc& L, bool pot);
 struct AxisInfo {
     int64_t passes, launches, chain_x, chain_y, seg_rows;
 };
+// Rows that arrive in pieces (ts_evolve_host: the host-to-device copy of rows [y_end[k-1],
+// y_end[k]) of both planes has completed when ready[k] has): the row chain of a piece starts as
+// soon as the piece is there, while the next one is still on the bus.
+struct RowFeed {
+    int n;
+    const int64_t* y_end;
+    const cudaEvent_t* ready;
+};
 bool axis_supported(const LatticeDesc& L, const StepCoef* pat, int period);
 bool axis_needs_scratch(const LatticeDesc& L);
 int axis_default_chain(const LatticeDesc& L);
@@ -146,7 +154,11 @@ int axis_default_chain(const LatticeDesc& L);
 // chain: sub-steps per windowed / pipelined pass (0 = default); seg_rows, nst: 0 = default.
 int axis_evolve(const LatticeDesc& L, void* psi_re, void* psi_im, void* scr_re, void* scr_im,
                 const StepCoef* pat, int period, int64_t n_sub, int chain, int seg_rows, int nst,
-                cudaStream_t st, AxisInfo* info, LaunchTimer* timer = nullptr);
+                cudaStream_t st, AxisInfo* info, LaunchTimer* timer = nullptr,
+                const RowFeed* feed = nullptr);
+// true if axis_evolve consumes a RowFeed piece by piece on this lattice (rows resident in
+// registers); otherwise the caller waits for the last piece before the call
+bool axis_takes_feed(const LatticeDesc& L);
 
 
 // ---- three-dimensional lattices ------------------------------------------------------------------------
