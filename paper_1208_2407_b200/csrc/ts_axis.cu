@@ -868,7 +868,7 @@ ycol_kernel(const __grid_constant__ YcolParams<T> p
 ) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr uint32_t ROWB = kYCols * sizeof(T);
-    constexpr uint32_t SLOTB = 4 * ROWB;          // re0 im0 re1 im1
+    constexpr uint32_t SLOTB = 8 * ROWB;          // two row pairs: re0 re1 im0 im1, twice
 
     const int lane = threadIdx.x & 31;
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
@@ -912,120 +912,108 @@ ycol_kernel(const __grid_constant__ YcolParams<T> p
     asm volatile("griddepcontrol.wait;" ::: "memory");
     asm volatile("griddepcontrol.launch_dependents;");
 
-    // running fetch position (warp-uniform): rows (fy, fy+1) of the strip's columns
+    // running fetch position (warp-uniform): rows (fy, fy+1) and (fy+2, fy+3) of the strip's columns
     int fy = PERY ? rows::wrap_index(y_in0, p.ny) : y_in0;
     uint32_t f_dst = ring, f_bar = bars;
     int f_slot = 0;
-#if TS_YCOL_TMAP
-    // One tensor-map copy per plane and iteration: the box is 32 columns x 2 rows at element
-    // coordinates (x0c, fy) -- no 64-bit address arithmetic in the loop (the four 1-D bulk copies
-    // per iteration cost ~38 uniform-datapath instructions of 180, ncu r2), columns beyond the
-    // lattice arrive as zeros.  Slot layout: re row 0, re row 1, im row 0, im row 1.
+    // A ring slot holds the row pairs of TWO iterations (the loop body below is two iterations long)
+    // and has ONE mbarrier: the slot counters, the barrier arithmetic and the refill test are paid
+    // once per body, not once per iteration (they were ~23 of the 168 instructions of an
+    // iteration).  Per pair and plane one tensor-map copy: the box is 32 columns x 2 rows at
+    // element coordinates (x0c, y) -- no 64-bit address arithmetic in the loop, columns beyond the
+    // lattice arrive as zeros, and the second pair wraps on its own on a periodic lattice.
+    // Slot layout: pair A = re row 0, re row 1, im row 0, im row 1; pair B the same, 4 rows on.
     (void)bytes;
-    auto issue = [&]() {
-        const bool rowok = PERY || (fy >= 0 && fy < p.ny);
+    auto issue = [&](auto edge_tag) {
+        // (only the warps of the edge variant ever fetch rows beyond a closed lattice)
+        constexpr bool EDGE = decltype(edge_tag)::value;
+        int fy2 = fy + 2;
+        if (PERY && fy2 >= p.ny) fy2 -= p.ny;
+        const bool ok1 = !EDGE || (fy >= 0 && fy < p.ny);
+        const bool ok2 = !EDGE || (fy2 >= 0 && fy2 < p.ny);
         if (leader) {
-            if (rowok) {
-                mbar_arrive_expect_tx(f_bar, 4 * ROWB);
-                tensor2d_g2s(f_dst, &tm_re, x0c, fy, f_bar);
-                tensor2d_g2s(f_dst + 2 * ROWB, &tm_im, x0c, fy, f_bar);
+            if (ok1 || ok2) {
+                mbar_arrive_expect_tx(f_bar, ((ok1 ? 4u : 0u) + (ok2 ? 4u : 0u)) * ROWB);
+                if (ok1) {
+                    tensor2d_g2s(f_dst, &tm_re, x0c, fy, f_bar);
+                    tensor2d_g2s(f_dst + 2 * ROWB, &tm_im, x0c, fy, f_bar);
+                }
+                if (ok2) {
+                    tensor2d_g2s(f_dst + 4 * ROWB, &tm_re, x0c, fy2, f_bar);
+                    tensor2d_g2s(f_dst + 6 * ROWB, &tm_im, x0c, fy2, f_bar);
+                }
             } else {
                 mbar_arrive(f_bar);
             }
         }
-        fy += 2;
+        fy = fy2 + 2;
         if (PERY && fy >= p.ny) fy -= p.ny;
         f_dst += SLOTB; f_bar += 8;
         if (++f_slot == NST) { f_slot = 0; f_dst = ring; f_bar = bars; }
     };
     constexpr uint32_t kOffAim = 2 * ROWB, kOffBre = ROWB;      // a = row 0, b = row 1 of the pair
-#else
-    const int64_t pitchB = (int64_t)p.nx * sizeof(T);
-    const int64_t planeB = pitchB * p.ny;
-    const char* f_re = reinterpret_cast<const char*>(p.src_re + x0c) + (int64_t)fy * pitchB;
-    const char* f_im = reinterpret_cast<const char*>(p.src_im + x0c) + (int64_t)fy * pitchB;
-    auto issue = [&]() {
-        const bool rowok = PERY || (fy >= 0 && fy < p.ny);
-        if (leader) {
-            if (rowok) {
-                mbar_arrive_expect_tx(f_bar, 4 * bytes);
-                bulk_g2s(f_dst, f_re, bytes, f_bar);
-                bulk_g2s(f_dst + ROWB, f_im, bytes, f_bar);
-                bulk_g2s(f_dst + 2 * ROWB, f_re + pitchB, bytes, f_bar);
-                bulk_g2s(f_dst + 3 * ROWB, f_im + pitchB, bytes, f_bar);
-            } else {
-                mbar_arrive(f_bar);
-            }
-        }
-        fy += 2; f_re += 2 * pitchB; f_im += 2 * pitchB;
-        if (PERY && fy >= p.ny) { fy -= p.ny; f_re -= planeB; f_im -= planeB; }
-        f_dst += SLOTB; f_bar += 8;
-        if (++f_slot == NST) { f_slot = 0; f_dst = ring; f_bar = bars; }
-    };
-    constexpr uint32_t kOffAim = ROWB, kOffBre = 2 * ROWB;      // re0 im0 re1 im1
-#endif
-    // the ring is filled completely; iteration i lives in slot i mod NST and is refilled, for
-    // iteration i + NST, at the top of iteration i + 1 (when its values have been consumed)
-    for (int k = 0; k < NST; ++k)
-        if (k < n_iter) issue();
-
+    // the ring is filled completely; body b (iterations 2b, 2b+1) lives in slot b mod NST, which is
+    // refilled for body b + NST in the middle of body b (when both its pairs are in registers)
     auto run = [&](auto edge_tag) {
         constexpr bool EDGE = decltype(edge_tag)::value;
+        for (int k = 0; k < NST; ++k)
+            if (2 * k < n_iter) issue(edge_tag);
         Cx<T> W[S][2][2];
 #pragma unroll
         for (int s = 0; s < S; ++s)
 #pragma unroll
             for (int a = 0; a < 4; ++a) { W[s][a >> 1][a & 1].re = T(0); W[s][a >> 1][a & 1].im = T(0); }
-        // software pipeline over the ring: while iteration i is computed, the row pair of
-        // iteration i+1 is read from its slot (known complete) and the barrier of iteration i+2 is
-        // tested; the blocking wait on it comes after the arithmetic has been issued
-        uint32_t l_src = ring + lane_off, l_bar = bars, l_ph = 0;      // slot of iteration i + 1
-        int l_slot = 0;
-        auto advance = [&]() {
-            l_src += SLOTB; l_bar += 8;
-            if (++l_slot == NST) { l_slot = 0; l_src = ring + lane_off; l_bar = bars; l_ph ^= 1; }
-        };
-        auto fetch_regs = [&](int y, Cx<T>& a, Cx<T>& b) {
+        // software pipeline over the ring: in the first half of body b pair A (read during the
+        // previous body) is computed while pair B is read from the same slot and the barrier of
+        // slot b+1 is tested (the blocking wait comes after the arithmetic has been issued); in
+        // the second half the slot is handed back for refilling, pair A of body b+1 is read from
+        // the next slot and pair B is computed
+        uint32_t c_src = ring + lane_off;                       // slot of body b
+        uint32_t n_src = c_src + SLOTB, n_bar = bars + 8, n_ph = 0;      // slot of body b + 1
+        int n_slot = 1;
+        if (NST == 1) { n_src = c_src; n_bar = bars; n_ph = 1; n_slot = 0; }
+        auto fetch_regs = [&](uint32_t src, int y, Cx<T>& a, Cx<T>& b) {
             const bool rowok = !EDGE || (y >= 0 && y < p.ny);
             if (rowok) {
-                a.re = lds1(l_src, T()); a.im = lds1(l_src + kOffAim, T());
-                b.re = lds1(l_src + kOffBre, T()); b.im = lds1(l_src + 3 * ROWB, T());
+                a.re = lds1(src, T()); a.im = lds1(src + kOffAim, T());
+                b.re = lds1(src + kOffBre, T()); b.im = lds1(src + 3 * ROWB, T());
             } else {
                 a.re = a.im = b.re = b.im = T(0);
             }
         };
         Cx<T> xa[2], xb[2];
-        mbar_wait(l_bar, l_ph);
-        fetch_regs(y_in0, xa[0], xa[1]);
-        advance();
-        if (1 < n_iter) mbar_wait(l_bar, l_ph);     // n_iter is even and >= 2
+        mbar_wait(bars, 0);
+        fetch_regs(c_src, y_in0, xa[0], xa[1]);
         int y = y_in0;
         T* o_re = p.dst_re + (int64_t)(y_in0 - 2 * S) * p.nx + x0c + lane;
         T* o_im = p.dst_im + (int64_t)(y_in0 - 2 * S) * p.nx + x0c + lane;
+        auto stages = [&](auto utag, int it, Cx<T> (&cur)[2]) {
+            constexpr int U = decltype(utag)::value;
+            Cx<T> x0 = cur[0], x1 = cur[1];
+            YStages<T, S, EDGE, UNI, 0>::run(p, y, W, U, x0, x1);
+            if (it >= 2 * S && lane_ok && y - 2 * S < y_out1) {
+                mulc(x0, p.out_scale); mulc(x1, p.out_scale);
+                o_re[0] = x0.re; o_im[0] = x0.im;
+                o_re[p.nx] = x1.re; o_im[p.nx] = x1.im;
+            }
+            y += 2; o_re += 2 * (int64_t)p.nx; o_im += 2 * (int64_t)p.nx;
+        };
 #pragma unroll 1
         for (int it0 = 0; it0 < n_iter; it0 += 2) {
-            auto half = [&](auto utag, Cx<T> (&cur)[2], Cx<T> (&nxt)[2]) {
-                constexpr int U = decltype(utag)::value;
-                const int it = it0 + U;
-                __syncwarp();      // every lane has consumed the slot of iteration it - 1
-                if (it >= 1 && it - 1 + NST < n_iter) issue();
-                // slot of iteration it + 1: complete (waited for below, one iteration ago)
-                if (it + 1 < n_iter) fetch_regs(y + 2, nxt[0], nxt[1]);
-                advance();
-                bool ready = true;
-                if (it + 2 < n_iter) ready = mbar_test(l_bar, l_ph);
-                Cx<T> x0 = cur[0], x1 = cur[1];
-                YStages<T, S, EDGE, UNI, 0>::run(p, y, W, U, x0, x1);
-                if (it >= 2 * S && lane_ok && y - 2 * S < y_out1) {
-                    mulc(x0, p.out_scale); mulc(x1, p.out_scale);
-                    o_re[0] = x0.re; o_im[0] = x0.im;
-                    o_re[p.nx] = x1.re; o_im[p.nx] = x1.im;
-                }
-                y += 2; o_re += 2 * (int64_t)p.nx; o_im += 2 * (int64_t)p.nx;
-                if (!ready) mbar_wait(l_bar, l_ph);
-            };
-            half(std::integral_constant<int, 0>{}, xa, xb);
-            half(std::integral_constant<int, 1>{}, xb, xa);
+            // ---- first half: pair A
+            fetch_regs(c_src + 4 * ROWB, y + 2, xb[0], xb[1]);       // n_iter is even
+            bool ready = true;
+            if (it0 + 2 < n_iter) ready = mbar_test(n_bar, n_ph);
+            stages(std::integral_constant<int, 0>{}, it0, xa);
+            if (!ready) mbar_wait(n_bar, n_ph);
+            // ---- second half: pair B
+            __syncwarp();      // every lane has both pairs of this slot in registers
+            if (it0 + 2 * NST < n_iter) issue(edge_tag);
+            if (it0 + 2 < n_iter) fetch_regs(n_src, y + 2, xa[0], xa[1]);
+            c_src = n_src;
+            n_src += SLOTB; n_bar += 8;
+            if (++n_slot == NST) { n_slot = 0; n_src = ring + lane_off; n_bar = bars; n_ph ^= 1; }
+            stages(std::integral_constant<int, 1>{}, it0 + 1, xb);
         }
     };
     const bool edge = !PERY && (y_in0 < 0 || y_in0 + 2 * n_iter >= p.ny);
@@ -1435,7 +1423,7 @@ int plane_map(CUtensorMap* m, const T* plane, int nx, int ny) {
 
 template <typename T, int S, bool PERY, bool UNI>
 int launch_ycol(const YcolParams<T>& p, cudaStream_t st) {
-    constexpr uint32_t SLOTB = 4 * kYCols * sizeof(T);
+    constexpr uint32_t SLOTB = 8 * kYCols * sizeof(T);
     const size_t smem = (size_t)kYWarps * p.nst * (SLOTB + 8);
     auto kern = ycol_kernel<T, S, PERY, UNI>;
     static std::atomic<size_t> configured[64];
@@ -1725,8 +1713,9 @@ static int axis_evolve_t(const LatticeDesc& L, T* psi_re, T* psi_im, T* scr_re, 
     } else {
         // ring slots per warp: at least 3 (iteration i+2 is waited for while slot i-1 is the one
         // being refilled), at most what 200 KB of shared memory per block hold
-        int slots = nst >= 3 ? nst : (nst > 0 ? 3 : 8);
-        const int slot_max = (int)((200 << 10) / (kYWarps * (4 * kYCols * sizeof(T) + 8)));
+        // (nst counts row pairs, as for the tile kernel; a ring slot holds two)
+        int slots = nst >= 3 ? (nst + 1) / 2 : (nst > 0 ? 2 : 4);
+        const int slot_max = (int)((200 << 10) / (kYWarps * (8 * kYCols * sizeof(T) + 8)));
         if (slots > slot_max) slots = slot_max;
         StepCoef subs[kMaxChain];
         int64_t i = 0;
