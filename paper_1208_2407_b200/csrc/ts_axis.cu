@@ -17,8 +17,8 @@
 //
 //   line_kernel   a WHOLE line (row or column) lives in registers for the complete chain -- all n
 //                 sub-steps in ONE launch, the state read once and written once: NS consecutive
-//                 sites per lane, 32 lanes per warp, up to 16 warps per line (16384 sites in fp32,
-//                 8192 in fp64).  In-thread pairs are plain FMAs, one pair per lane and odd sweep
+//                 sites per lane (2..32; 64 for some fp32 rows), 32 lanes per warp, up to 16 warps
+//                 per line (16384 sites in fp32, 8192 in fp64).  In-thread pairs are plain FMAs, one pair per lane and odd sweep
 //                 crosses lanes by shuffle, one pair per warp crosses warps through 16 bytes of
 //                 shared memory and an mbarrier per line (arrive after the even sweep, wait after
 //                 the in-thread odd pairs).  No halo, no passes, no redundant work.
@@ -27,8 +27,9 @@
 //                 n <= 24 sub-steps per pass.
 //   ycol_kernel   long COLUMNS: a streaming register pipeline -- a warp walks down a strip of 32
 //                 columns, one per lane, S <= 24 chained sub-steps in flight, rows brought in by
-//                 bulk async copies (TMA) into a per-warp shared-memory ring.  No x halo at all;
-//                 4S warm-up rows per segment.
+//                 2-D tensor-map copies (TMA, cp.async.bulk.tensor.2d) into a per-warp shared-memory
+//                 ring whose slots hold the row pairs of two iterations under one mbarrier.  No x
+//                 halo at all; 4S warm-up rows per segment.
 //   tline_kernel  strided lines of a state that does not stay in L2 (y and z of a 3-D lattice):
 //                 one LANE per line, 32 adjacent lines per warp (coalesced rows), the line cut
 //                 over the warps of the block.
@@ -54,9 +55,6 @@
 #include "ts_rows.cuh"
 #include "ts_tma.cuh"
 
-#ifndef TS_YCOL_TMAP
-#define TS_YCOL_TMAP 1      // column pipeline: rows fetched by 2-D tensor-map copies (0: 1-D bulk copies)
-#endif
 
 namespace ts {
 namespace {
@@ -861,11 +859,8 @@ constexpr int ycol_min_blocks() {
 
 template <typename T, int S, bool PERY, bool UNI>
 __global__ void __launch_bounds__(kYWarps * 32, ycol_min_blocks<T, S, UNI>())
-ycol_kernel(const __grid_constant__ YcolParams<T> p
-#if TS_YCOL_TMAP
-            , const __grid_constant__ CUtensorMap tm_re, const __grid_constant__ CUtensorMap tm_im
-#endif
-) {
+ycol_kernel(const __grid_constant__ YcolParams<T> p, const __grid_constant__ CUtensorMap tm_re,
+            const __grid_constant__ CUtensorMap tm_im) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr uint32_t ROWB = kYCols * sizeof(T);
     constexpr uint32_t SLOTB = 8 * ROWB;          // two row pairs: re0 re1 im0 im1, twice
@@ -1384,7 +1379,6 @@ int xwin_pass(const LatticeDesc& L, const T* src_re, const T* src_im, T* dst_re,
     return TS_OK;
 }
 
-#if TS_YCOL_TMAP
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
                                   const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
@@ -1419,7 +1413,6 @@ int plane_map(CUtensorMap* m, const T* plane, int nx, int ny) {
     if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled failed"); return TS_ECUDA; }
     return TS_OK;
 }
-#endif
 
 template <typename T, int S, bool PERY, bool UNI>
 int launch_ycol(const YcolParams<T>& p, cudaStream_t st) {
@@ -1448,15 +1441,11 @@ int launch_ycol(const YcolParams<T>& p, cudaStream_t st) {
     cfg.attrs = attr;
     // as in ts_stream.cu: dependent launch only for grids of at most one wave
     cfg.numAttrs = ((int64_t)grid.x * grid.y <= (int64_t)sm_count() * ycol_min_blocks<T, S, UNI>()) ? 1 : 0;
-#if TS_YCOL_TMAP
     alignas(64) CUtensorMap tm_re, tm_im;
     int rc = plane_map<T>(&tm_re, p.src_re, p.nx, p.ny);
     if (rc == TS_OK) rc = plane_map<T>(&tm_im, p.src_im, p.nx, p.ny);
     if (rc != TS_OK) return rc;
     TS_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, p, tm_re, tm_im));
-#else
-    TS_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, p));
-#endif
     return TS_OK;
 }
 
