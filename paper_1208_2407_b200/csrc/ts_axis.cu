@@ -353,10 +353,10 @@ __device__ __forceinline__ void phase_mul(Cx<T>& s, T pr, T pi) {
     s.im = fma(m, pr, r * pi);
 }
 
-// Boundary-site exchange between the warps of one line, branch-free: lane 0 / lane 31 store and
-// load their site under a predicate (an `if` around them costs two
-// divergent branches and a reconvergence per sub-step; ncu: branch_resolving was the top stall of
-// the 16-warp kernel).
+// Shared-memory accesses of the exchange between the lanes of a line, as inline PTX under a
+// predicate (the line kernel passes `true` and ptxas drops it; with a per-lane predicate they are
+// the branch-free form of `if (lane == 0) ...`, which as an `if` cost two divergent branches and a
+// reconvergence per sub-step -- ncu, r2d: branch_resolving was the top stall of the 16-warp kernel).
 __device__ __forceinline__ void st_if(bool pred, uint32_t addr, const Cx<float>& v) {
     asm volatile(
         "{\n\t"
@@ -414,13 +414,16 @@ __global__ void __launch_bounds__(MW ? (sizeof(T) * NS >= 256 ? 256 : 512) : 128
                                   MW ? 1 : (sizeof(T) * NS >= 128 ? 3 : 4))
 line_kernel(const __grid_constant__ LineParams<T> p) {
     constexpr int PW = (Piece<T>::n < NS) ? Piece<T>::n : NS;     // sites per vector access
-    // Exchange of the pair that straddles two warps of a line: entry b (b = the block's warp index
-    // of the warp AFTER the cut) holds {first site of warp b, last site of warp b - 1}, twice
-    // (parity sets used by alternate sub-steps), and the line has ONE mbarrier that every warp
-    // arrives on after publishing.  (Measured alternative, r2g: neighbour-to-neighbour barriers --
-    // two arrivals and two waits per warp and sub-step, warps free to drift apart by a sub-step --
-    // C4 rows 10.97 ms against 9.22 ms with the line-wide barrier.)
-    __shared__ __align__(16) Cx<T> xbuf[2][MW ? kMaxLineWarps : 1][2];
+    // Exchange between the lanes of a line that several warps share: every thread publishes its
+    // first and its last site in shared memory (two parity sets, used by alternate sub-steps) and
+    // reads its two neighbours' from there -- no shuffles, nothing predicated on the lane -- and
+    // the line has ONE mbarrier that every warp arrives on after publishing.  (Before, r2: shuffles
+    // inside a warp and only the pair that straddles two warps through shared memory, by
+    // predicated accesses of lanes 0 / 31: 110 instructions per sub-step against 101, C4 rows
+    // 8.55 ms against 8.26.  Measured alternative, r2g: neighbour-to-neighbour barriers -- two
+    // arrivals and two waits per warp and sub-step, warps free to drift apart by a sub-step -- C4
+    // rows 10.97 ms against 9.22 ms with the line-wide barrier.)
+    __shared__ __align__(16) Cx<T> xs[2][2][MW ? 512 : 1];      // [parity set][first | last][thread]
     __shared__ __align__(8) uint64_t xbar[MW ? kMaxLineWarps : 1];
 
     const int lane = threadIdx.x & 31;
@@ -434,15 +437,22 @@ line_kernel(const __grid_constant__ LineParams<T> p) {
         __syncthreads();
     }
     const uint32_t bar = smem_u32(&xbar[MW ? grp : 0]);
-    uint32_t ph = 0, par = 0;
-    constexpr uint32_t kParB = (MW ? kMaxLineWarps : 1) * 2 * sizeof(Cx<T>);
-    const bool is_first = lane == 0, is_last = lane == 31;
-    const int w_dn = MW ? grp * W + (wl == W - 1 ? 0 : wl + 1) : 0;     // entry after this warp
-    const int w_me = MW ? grp * W + wl : 0;                             // entry before this warp
-    const int bnd = is_last ? w_dn : w_me;
-    // lane 0 writes its entry's first half and reads the second; lane 31 the other way round
-    const uint32_t xb_st = smem_u32(&xbuf[0][bnd][is_last ? 1 : 0]);
-    const uint32_t xb_ld = smem_u32(&xbuf[0][bnd][is_last ? 0 : 1]);
+    uint32_t ph = 0;
+    const bool is_first = lane == 0;
+    // the threads of a line are consecutive in the block; its ends close on each other (a closed
+    // line ignores what it reads there)
+    const int t_line0 = MW ? grp * W * 32 : 0;
+    const int t_me = MW ? (int)threadIdx.x : 0;
+    const int t_up = MW ? (t_me == t_line0 ? t_line0 + W * 32 - 1 : t_me - 1) : 0;
+    const int t_dn = MW ? (t_me == t_line0 + W * 32 - 1 ? t_line0 : t_me + 1) : 0;
+    // one running address (own `first` slot of the current parity set); everything else is a
+    // constant distance from it: own `last` slot (immediate), the upper neighbour's `last`, the
+    // lower neighbour's `first` (two per-thread constants: the ends of a line differ)
+    constexpr uint32_t kWhichX = (MW ? 512 : 1) * sizeof(Cx<T>);
+    constexpr uint32_t kParX = 2 * kWhichX;
+    uint32_t sx = smem_u32(&xs[0][0][t_me]);
+    const uint32_t d_up = kWhichX + (uint32_t)((t_up - t_me) * (int)sizeof(Cx<T>));
+    const uint32_t d_dn = (uint32_t)((t_dn - t_me) * (int)sizeof(Cx<T>));
 
     const int xl = (wl * 32 + lane) * NS;       // first site of the lane
     const bool active = MW || lane < p.n_lanes;
@@ -487,34 +497,27 @@ line_kernel(const __grid_constant__ LineParams<T> p) {
 
         auto xbegin = [&](Line<T, NS>& M, Cx<T>& up, Cx<T>& dn) {
             if (MW) {
-                // publish the boundary sites (state after the even sweep); the wait for the
-                // neighbouring warps' comes after the in-thread work
-                st_if(is_first, xb_st + par, M.s[0]);
-                st_if(is_last, xb_st + par, M.s[NS - 1]);
+                // publish the two outer sites (state after the even sweep); the wait for the
+                // neighbours' comes after the in-thread work
+                st_if(true, sx, M.s[0]);
+                st_if(true, sx + kWhichX, M.s[NS - 1]);
                 __syncwarp();
                 if (is_first) mbar_arrive(bar);
+                return;
             }
-            if (MW) {
-                // neighbouring lanes by a constant distance (no index arithmetic in the loop);
-                // lanes 0 / 31 get their own value back and take the other warp's in xend
-                up.re = __shfl_up_sync(0xffffffffu, M.s[NS - 1].re, 1);
-                up.im = __shfl_up_sync(0xffffffffu, M.s[NS - 1].im, 1);
-                dn.re = __shfl_down_sync(0xffffffffu, M.s[0].re, 1);
-                dn.im = __shfl_down_sync(0xffffffffu, M.s[0].im, 1);
-            } else {
-                up.re = __shfl_sync(0xffffffffu, M.s[NS - 1].re, up_src);
-                up.im = __shfl_sync(0xffffffffu, M.s[NS - 1].im, up_src);
-                dn.re = __shfl_sync(0xffffffffu, M.s[0].re, dn_src);
-                dn.im = __shfl_sync(0xffffffffu, M.s[0].im, dn_src);
-            }
+            // one warp per line: the ring of lanes by shuffles
+            up.re = __shfl_sync(0xffffffffu, M.s[NS - 1].re, up_src);
+            up.im = __shfl_sync(0xffffffffu, M.s[NS - 1].im, up_src);
+            dn.re = __shfl_sync(0xffffffffu, M.s[0].re, dn_src);
+            dn.im = __shfl_sync(0xffffffffu, M.s[0].im, dn_src);
         };
         auto xend = [&](Cx<T>& up, Cx<T>& dn) {
             if (MW) {
                 mbar_wait_bounded(bar, ph);
                 ph ^= 1;
-                ld_if(is_first, xb_ld + par, up);
-                ld_if(is_last, xb_ld + par, dn);
-                par ^= kParB;
+                ld_if(true, sx + d_up, up);
+                ld_if(true, sx + d_dn, dn);
+                sx ^= kParX;
             }
         };
         if (p.n_prog == 0) {
