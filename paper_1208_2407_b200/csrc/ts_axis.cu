@@ -417,7 +417,8 @@ line_kernel(const __grid_constant__ LineParams<T> p) {
     // Exchange between the lanes of a line that several warps share: every thread publishes its
     // first and its last site in shared memory (two parity sets, used by alternate sub-steps) and
     // reads its two neighbours' from there -- no shuffles, nothing predicated on the lane -- and
-    // the line has ONE mbarrier that every warp arrives on after publishing.  (Before, r2: shuffles
+    // the line has ONE mbarrier that every THREAD arrives on after publishing (its own stores are
+    // ordered before its own arrival: no __syncwarp, no elected lane; C4 rows 8.27 -> 8.17 ms).  (Before, r2: shuffles
     // inside a warp and only the pair that straddles two warps through shared memory, by
     // predicated accesses of lanes 0 / 31: 110 instructions per sub-step against 101, C4 rows
     // 8.55 ms against 8.26.  Measured alternative, r2g: neighbour-to-neighbour barriers -- two
@@ -432,13 +433,12 @@ line_kernel(const __grid_constant__ LineParams<T> p) {
     const int wl = MW ? warp % W : 0;           // this warp's place in its line
     const int grp = MW ? warp / W : warp;       // the line of the block this warp belongs to
     if (MW) {
-        if (threadIdx.x < p.lines_per_block) mbar_init(smem_u32(&xbar[threadIdx.x]), W);
+        if (threadIdx.x < p.lines_per_block) mbar_init(smem_u32(&xbar[threadIdx.x]), W * 32);
         mbar_fence_init();
         __syncthreads();
     }
     const uint32_t bar = smem_u32(&xbar[MW ? grp : 0]);
     uint32_t ph = 0;
-    const bool is_first = lane == 0;
     // the threads of a line are consecutive in the block; its ends close on each other (a closed
     // line ignores what it reads there)
     const int t_line0 = MW ? grp * W * 32 : 0;
@@ -501,8 +501,7 @@ line_kernel(const __grid_constant__ LineParams<T> p) {
                 // neighbours' comes after the in-thread work
                 st_if(true, sx, M.s[0]);
                 st_if(true, sx + kWhichX, M.s[NS - 1]);
-                __syncwarp();
-                if (is_first) mbar_arrive(bar);
+                mbar_arrive(bar);      // every thread: its own stores are ordered before its arrival
                 return;
             }
             // one warp per line: the ring of lanes by shuffles
