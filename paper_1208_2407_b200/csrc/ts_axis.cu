@@ -1271,16 +1271,16 @@ int launch_lines(const LineGeom& g, int dtype, LineParams<T>& p, T* re, T* im, c
     }
     LineShape sh = line_shape(g.n_sites, dtype);
     if (!sh.ok()) { set_error("axis: line does not fit a thread block"); return TS_EUNSUPPORTED; }
-    // long fp32 rows: 64 sites per lane and half the warps -- the per-sub-step cost of the exchange
-    // (publish, arrive, wait, pick up: ~45 instructions per warp) is spread over twice the sites,
-    // at 255 registers, i.e. 8 warps per SM.  Taken where those 8 warps are whole lines of 2, 4 or
-    // 8 warps and it measured faster (200 sub-steps, rows only, ms, 32 -> 64 sites per lane):
-    // 4096^2 0.600 -> 0.580 / closed 0.648 -> 0.582, 8192^2 2.35 -> 2.30 / closed 2.60 -> 2.31,
-    // 16384^2 closed 9.51 -> 9.06; NOT for periodic rows of 16384 (one line of 8 warps per SM:
-    // 8.53 -> 8.86) nor where the warps do not fill the SM (12288: 1.76 -> 2.12).
+    // fp32 rows of 4096 / 8192 sites: 64 sites per lane and half the warps -- the per-sub-step
+    // cost of the exchange (~32 instructions per warp) is spread over twice the sites, at 255
+    // registers, i.e. 8 warps per SM in whole lines of 2 or 4 warps.  Measured with the final
+    // exchange (200 sub-steps, rows only, ms, 32 -> 64 sites per lane): 4096^2 0.549 -> 0.537 /
+    // closed 0.582 -> 0.541, 8192^2 2.20 -> 2.13 / closed 2.31 -> 2.13; NOT for rows of 16384 (one
+    // line of 8 warps per SM cannot hide its own barrier: closed 8.57 -> 8.75; periodic, with the
+    // earlier exchange, 8.53 -> 8.86) nor
+    // where the warps do not fill the SM (12288: 1.76 -> 2.12).
     static const bool ns64 = getenv("TS_PROBE_NO_NS64") == nullptr;
-    if (ns64 && !g.col && dtype == TS_F32 && sh.ns == 32 &&
-        (sh.warps == 4 || sh.warps == 8 || (sh.warps == 16 && !g.periodic))) {
+    if (ns64 && !g.col && dtype == TS_F32 && sh.ns == 32 && (sh.warps == 4 || sh.warps == 8)) {
         sh.ns = 64;
         sh.warps /= 2;
     }

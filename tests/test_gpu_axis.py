@@ -51,8 +51,8 @@ def test_resident_lines(dtype, boundary, idx, n_steps):
     assert info["chain_x"] == n_steps and info["chain_y"] == n_steps
 
 
-# lines shared by several warps of a block (2048 = 2 x 32 x 32, 1152 = 9 x 32 x 4, 4096 / 8192 /
-# closed 16384 in fp32 = 2 / 4 / 8 warps of 64 sites per lane, ...), rows that
+# lines shared by several warps of a block (2048 = 2 x 32 x 32, 1152 = 9 x 32 x 4, 4096 / 8192 in
+# fp32 = 2 / 4 warps of 64 sites per lane, 16384 = 16 warps of 32, ...), rows that
 # fit no block and are cut into windows with a halo (1056 = 33 x 32, 20480, 528, 12288), columns
 # that are pipelined (130, 1100, 66 rows: no lane layout divides them)
 LONG = {"f32": [(2048, 128), (1152, 200), (64, 2048), (1280, 130), (3072, 1100), (4096, 66),
