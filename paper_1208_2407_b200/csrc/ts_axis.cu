@@ -586,7 +586,7 @@ tline_kernel(const __grid_constant__ LineParams<T> p) {
     const int lane = threadIdx.x & 31;
     const int w = threadIdx.x >> 5;
     const int W = p.n_warps;
-    if (threadIdx.x == 0) mbar_init(smem_u32(&xbar), W);
+    if (threadIdx.x == 0) mbar_init(smem_u32(&xbar), W * 32);
     mbar_fence_init();
     __syncthreads();
     const uint32_t bar = smem_u32(&xbar);
@@ -595,7 +595,6 @@ tline_kernel(const __grid_constant__ LineParams<T> p) {
     const int wu = w == 0 ? W - 1 : w - 1, wd = w == W - 1 ? 0 : w + 1;
     const bool cut_up = EDGE && !p.periodic && w == 0;
     const bool cut_dn = EDGE && !p.periodic && w == W - 1;
-    const bool leader = lane == 0;
 
     for (int64_t l0 = (int64_t)blockIdx.x * 32; l0 < p.n_lines; l0 += (int64_t)gridDim.x * 32) {
         const int64_t line = l0 + lane;
@@ -619,8 +618,7 @@ tline_kernel(const __grid_constant__ LineParams<T> p) {
             if (W == 1) { up = M.s[NS - 1]; dn = M.s[0]; return; }     // the line closes on itself
             xbuf[par][w][0][lane] = M.s[0];
             xbuf[par][w][1][lane] = M.s[NS - 1];
-            __syncwarp();
-            if (leader) mbar_arrive(bar);
+            mbar_arrive(bar);      // every thread, as in line_kernel: own stores before own arrival
         };
         auto xend = [&](Cx<T>& up, Cx<T>& dn) {
             if (W == 1) return;
