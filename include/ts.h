@@ -272,7 +272,9 @@ int ts_evolve_host(ts_plan* plan, void* psi_re_host, void* psi_im_host,
  *   "chain"        axis-split path: sub-steps per windowed / pipelined pass (<= 24 fp32, 12 fp64),
  *                  0 = auto.
  *   "ring_slots"   row-pair slots of the TMA ring per warp, 0 = auto (with phase planes: slots of the
- *                  state ring, i.e. prefetch distance + 1; the phase ring follows from it).
+ *                  state ring, i.e. prefetch distance + 1; the phase ring follows from it; the
+ *                  column pipeline of the axis-split path holds two row pairs per slot and rounds
+ *                  the count up to whole slots, at least two).
  *   "timing"       1: record CUDA events around every launch (ts_plan_get_launch_times), 0 = off.
  * Environment: TS_NO_PDL=1 turns off programmatic dependent launch between passes.
  */
